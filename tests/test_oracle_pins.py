@@ -1,0 +1,361 @@
+"""Pins for the FP64 oracle: each checks oracle/ against something other than
+itself -- published known answers, closed forms, brute force, textbook special cases, invariants."""
+import os
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads import generate as G
+from oracle import oracle as O
+from oracle.oracle import Oracle
+
+
+def _free(w):
+    """copy of w with the safe set = everything"""
+    import copy
+    v = copy.copy(w)
+    v.bidx = np.zeros(0, np.int32); v.blo = np.zeros(0, np.float32); v.bhi = np.zeros(0, np.float32)
+    v.annulus = 0
+    return v
+
+
+# ---------------------------------------------------------------- P8: sampler --------------------
+def test_philox_known_answers(golden_dir):
+    rows = [l.split() for l in open(os.path.join(golden_dir, "philox4x32_10_kat.txt")) if not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        assert O.philox4x32_10(v[0:4], v[4:6]) == v[6:10]
+
+
+def _py_philox(ctr, key):
+    """independent pure-Python restatement (Python ints) used to pin counter/key layout"""
+    M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
+    c = list(ctr); k = list(key)
+    for r in range(10):
+        if r:
+            k = [(k[0] + W0) & 0xFFFFFFFF, (k[1] + W1) & 0xFFFFFFFF]
+        p0, p1 = M0 * c[0], M1 * c[2]
+        c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xFFFFFFFF]
+    return c
+
+
+def test_philox_sampler_layout_and_mapping():
+    """counter = (i_lo, i_hi, tick_lo, tick_hi), key = (seed_lo, seed_hi), word j -> dim j,
+    r = (w>>8) 2^-24, u = fmaf(r, hi-lo, lo) in fp32 (DESIGN G4)."""
+    w = W.make("C5", calibrated=False)
+    w.seed = 0x1234_5678_9ABC_DEF0
+    w.u_lo = np.array([-1.0, 0.0, -1.0], np.float32); w.u_hi = np.array([1.0, 1.0, 0.0], np.float32)
+    o = Oracle(w)
+    tick = (7 << 32) | 99
+    idx = [0, 1, 2, 12345, w.N - 1]
+    got = o.sample(tick, idx)
+    for row, i in zip(got, idx):
+        words = _py_philox([i, 0, tick & 0xFFFFFFFF, tick >> 32], [w.seed & 0xFFFFFFFF, w.seed >> 32])
+        for j in range(3):
+            r = np.float32(words[j] >> 8) * np.float32(2.0 ** -24)
+            span = np.float32(w.u_hi[j] - w.u_lo[j])
+            exact = float(r) * float(span) + float(w.u_lo[j])          # fp64 is exact enough to round once
+            assert row[j] == np.float32(exact)
+            assert w.u_lo[j] <= row[j] <= w.u_hi[j]
+
+
+def test_philox_uniform_moments():
+    w = W.make("C1", calibrated=False)
+    o = Oracle(w, N=20000)
+    u = o.sample(3, np.arange(20000))[:, 0].astype(np.float64)
+    assert abs(u.mean()) < 0.02 and abs(u.var() - 1.0 / 3.0) < 0.01
+    assert u.min() >= -1 and u.max() <= 1
+    u2 = o.sample(4, np.arange(100))[:, 0]
+    assert not np.array_equal(u2, u[:100].astype(np.float32))        # fresh set each tick
+
+
+def test_grid_points_exact():
+    """endpoint-inclusive grid, row-major, dimension 0 slowest (DESIGN G3)."""
+    w = W.make("C3", calibrated=False)
+    o = Oracle(w)
+    u = o.sample(0, [0, 99, 100, 9999, 50 * 100 + 50])
+    assert tuple(u[0]) == (-1.0, -1.0) and tuple(u[1]) == (-1.0, 1.0)
+    assert u[2][1] == -1.0 and u[2][0] == np.float32(float(np.float32(1.0) / np.float32(99)) * 2.0 - 1.0)
+    assert tuple(u[3]) == (1.0, 1.0)
+    assert abs(u[4][0] - (-1 + 50 * 2 / 99)) < 1e-6
+    w.grid_counts = np.array([23, 1], np.int32); w.N = 23
+    u = Oracle(w).sample(0, np.arange(23))
+    assert u[11][0] == 0.0 and np.all(u[:, 1] == 0.0)                 # odd count contains "straight"
+    assert not np.array_equal(Oracle(w).sample(0, [5]), Oracle(w).sample(0, [6]))
+    assert np.array_equal(Oracle(w).sample(0, [5]), Oracle(w).sample(9, [5]))   # grid ignores tick
+
+
+# ---------------------------------------------------------------- P9: lift -----------------------
+def test_lift_hand_values():
+    w = W.make("C3", calibrated=False)
+    o = Oracle(w)
+    assert o.lift(np.zeros(6))[7] == 1.0 and np.count_nonzero(o.lift(np.zeros(6))) == 1   # only cos(0)
+    x = np.array([2.0, 3.0, 0.5, 5.0, 7.0, 11.0])
+    z = o.lift(x)
+    assert np.allclose(z[:6], x)
+    assert np.isclose(z[6], np.sin(0.5)) and np.isclose(z[7], np.cos(0.5))
+    prods = [x[i] * x[j] for i in range(6) for j in range(i, 6)]
+    assert np.allclose(z[8:29], prods)
+    assert np.allclose(z[29:], [5 * np.cos(0.5), 5 * np.sin(0.5), 7 * np.cos(0.5)])
+    w2 = W.make("C2", calibrated=False)
+    e1 = np.zeros(4); e1[1] = 2.0
+    z2 = Oracle(w2).lift(e1)
+    assert z2[1] == 2.0 and z2[14] == 8.0 and z2[15] == 0.0 and z2[8] == 4.0   # x1, x1^3, x3^3, x1*x1
+    assert np.count_nonzero(Oracle(w2).lift(np.zeros(4))) == 0
+
+
+def test_lift_rff_matches_numpy():
+    w = W.make("C5", calibrated=False)
+    x = np.linspace(-0.3, 0.4, 8)
+    z = Oracle(w).lift(x)
+    ref = w.scale * np.cos(w.W.astype(np.float64) @ x + w.b.astype(np.float64))
+    assert np.allclose(z[:8], x) and np.allclose(z[8:], ref, rtol=0, atol=1e-14)
+
+
+# ---------------------------------------------------------------- P1: closed forms ---------------
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5"])
+def test_rollout_closed_form(name):
+    """z_H = K^H z0 + sum_{k<H} K^k B u  (north_star) and (I-K)^-1 (I-K^H) B u  (rho(K) < 1)."""
+    w = _free(W.make(name, calibrated=False))
+    o = Oracle(w)
+    rng = np.random.default_rng(5)
+    K = w.K.astype(np.float64); B = w.B.astype(np.float64)
+    for _ in range(3):
+        z0 = o.lift(w.x_nom.astype(np.float64) + 0.01 * rng.standard_normal(w.n))
+        u = rng.uniform(-1, 1, w.m)
+        steps, _, traj = o.rollout(z0, u, want_traj=True)
+        assert steps == w.H
+        H = w.H
+        KH = np.linalg.matrix_power(K, H)
+        s = sum(np.linalg.matrix_power(K, k) @ B @ u for k in range(H))
+        zH = KH @ z0 + s
+        scale = max(np.linalg.norm(zH), 1e-12)
+        assert np.linalg.norm(traj[H - 1] - zH) / scale < 1e-10
+        geo = np.linalg.solve(np.eye(w.d) - K, (np.eye(w.d) - KH) @ B @ u)
+        assert np.linalg.norm(traj[H - 1] - (KH @ z0 + geo)) / scale < 1e-8
+        k = H // 3                                                   # an interior step too
+        zk = np.linalg.matrix_power(K, k + 1) @ z0 + sum(np.linalg.matrix_power(K, q) @ B @ u for q in range(k + 1))
+        assert np.linalg.norm(traj[k] - zk) / max(np.linalg.norm(zk), 1e-12) < 1e-10
+
+
+# ---------------------------------------------------------------- P2: brute force ----------------
+def _brute_tick(w, U, z0, u_h, H):
+    """un-vectorised Python restatement of Algorithm 2 l.2-13 with explicit sorting of key tuples"""
+    K = [[float(v) for v in row] for row in w.K]; B = [[float(v) for v in row] for row in w.B]
+    keys, steps_all = [], []
+    for i, u in enumerate(U):
+        z = [float(v) for v in z0]; steps = H
+        for k in range(H):
+            zn = []
+            for r in range(w.d):
+                s = 0.0
+                for c in range(w.d):
+                    s += K[r][c] * z[c]
+                for j in range(w.m):
+                    s += B[r][j] * float(u[j])
+                zn.append(s)
+            z = zn
+            ok = True
+            for q in range(len(w.bidx)):
+                v = z[int(w.bidx[q])]
+                ok = ok and (float(w.blo[q]) + float(w.inflate) < v < float(w.bhi[q]) - float(w.inflate))
+            if w.annulus:
+                r2 = (z[w.ix] - w.cx) ** 2 + (z[w.iy] - w.cy) ** 2
+                ok = ok and ((w.rmin + w.inflate) ** 2 <= r2 <= (w.rmax - w.inflate) ** 2)
+            if not ok:
+                steps = k
+                break
+        steps_all.append(steps)
+        dist = sum((float(u[j]) - float(u_h[j])) ** 2 for j in range(w.m)) ** 0.5
+        keys.append((0, dist, i) if steps == H else (1, H - steps, i))
+    return sorted(keys)[0], steps_all
+
+
+@pytest.mark.parametrize("name,shrink", [("C1", 1.0), ("C1", 0.05), ("C3", 1.0), ("C3", 0.02), ("C2", 1.0)])
+def test_tick_vs_brute_force(name, shrink):
+    w = W.make(name, calibrated=True, N=16, H=5)
+    if name == "C3":
+        w.grid_counts = np.array([4, 4], np.int32)
+    w = G.scaled_bounds(w, shrink)
+    w.inflate = 0.01
+    o = Oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 6)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        r = o.step(x0, uu, int(t), detail=True)
+        u_h = np.clip(uu, w.u_lo, w.u_hi)
+        key, steps_all = _brute_tick(w, r["U"], o.lift(x0.astype(np.float64)), u_h, w.H)
+        assert list(r["steps_all"]) == steps_all
+        assert r["index"] == key[2] and r["safe"] == (key[0] == 0)
+        assert r["n_safe"] == sum(s == w.H for s in steps_all)
+        assert r["n_exec"] == sum(min(s + 1, w.H) for s in steps_all)
+        if key[0] == 0:
+            assert abs(r["dist"] - key[1]) < 1e-15
+        else:
+            assert r["steps"] == w.H - key[1]
+    # the forced-fallback set really falls back, the literal set really has safe candidates
+    if shrink < 0.1:
+        assert r["safe"] == 0
+
+
+# ---------------------------------------------------------------- P3 / P4: invariants ------------
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5"])
+def test_minimal_intervention_and_membership(name):
+    """a safe u_user is returned unchanged; the selected input is a sampled one."""
+    w = W.make(name, N=512 if name != "C3" else 400)
+    if name == "C3":
+        w.grid_counts = np.array([20, 20], np.int32)
+    o = Oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 12)
+    seen_safe_user = seen_intervention = 0
+    for x0, uu, t in zip(x0s, uus, ticks):
+        r = o.step(x0, uu, int(t), detail=True)
+        assert 0 <= r["index"] <= w.N
+        assert np.array_equal(r["u"], r["U"][r["index"]])                       # P4
+        u_h = np.clip(uu, w.u_lo, w.u_hi)
+        assert np.array_equal(r["U"][w.N], u_h)
+        if r["steps_all"][w.N] == w.H:                                          # P3
+            seen_safe_user += 1
+            assert np.array_equal(r["u"], u_h) and r["dist"] == 0.0 and r["safe"] == 1
+            assert r["index"] == w.N or np.array_equal(r["U"][r["index"]], u_h)
+        elif r["safe"]:
+            seen_intervention += 1
+            assert r["dist"] > 0 and r["steps_all"][r["index"]] == w.H          # never an unsafe input
+    assert seen_safe_user > 0 and seen_intervention > 0
+
+
+# ---------------------------------------------------------------- P5: Eq. (2) --------------------
+def test_eq2_printed_value(golden_dir):
+    """1-D grid of 10,000 samples on [-1,1], everything safe, literal Alg. 2 (u_h not injected):
+    max deviation = half the spacing ~ lambda*/(2N) = 0.0001 as printed."""
+    row = [l.split() for l in open(os.path.join(golden_dir, "eq2_printed.txt")) if l.startswith("balance")][0]
+    lam, N, printed = float(row[1]), int(row[2]), float(row[3])
+    assert abs(lam / (2 * N) - printed) < 1e-12
+    w = _free(W.make("C1", calibrated=False, N=N, H=1))
+    w.sampler = 1; w.grid_counts = np.array([N], np.int32)
+    o = Oracle(w, include_user=0)
+    spacing = 2.0 / (N - 1)
+    worst = 0.0
+    rng = np.random.default_rng(0)
+    cells = rng.integers(0, N - 1, 40)
+    for c in cells:
+        for frac in (0.5, 0.25, 0.999):
+            u_h = np.float32(-1.0 + (c + frac) * spacing)
+            r = o.step(np.zeros(4, np.float32), np.array([u_h]), 0)
+            dev = abs(float(r["u"][0]) - float(u_h))
+            assert dev <= spacing / 2 + 2.0 ** -23                  # half the spacing (+ fp32 rounding of the grid)
+            worst = max(worst, dev)
+    assert worst > 0.99 * spacing / 2                                    # attained at cell mid-points
+    assert round(worst, 4) == printed
+
+
+# ---------------------------------------------------------------- P6: textbook special cases -----
+def test_special_case_K_zero():
+    """K = 0  =>  x_k = C B u for every k: safe iff that one point is in the safe set."""
+    w = W.make("C1", N=256, H=7)
+    w.K = np.zeros_like(w.K)
+    w.B = (w.B * 0 + np.linspace(0.2, 1.0, 8)[:, None]).astype(np.float32)
+    o = Oracle(w)
+    r = o.step(w.x_nom + 1.0, np.array([0.3], np.float32), 0, detail=True)
+    for i in range(w.N + 1):
+        x = w.B[:4, 0].astype(np.float64) * float(r["U"][i, 0])
+        ok = (-2 < x[0] < 2) and (-0.5 < x[1] < 0.5)
+        assert r["steps_all"][i] == (w.H if ok else 0)
+
+
+def test_special_case_K_rho_identity():
+    """K = rho I  =>  z_k = rho^k z0 + (1-rho^k)/(1-rho) B u ; first violation step in closed form."""
+    w = W.make("C1", N=300, H=40)
+    rho = 0.9
+    w.K = (rho * np.eye(8)).astype(np.float32)
+    w.B = np.zeros((8, 1), np.float32); w.B[1, 0] = 0.1
+    w.bidx = np.array([1], np.int32); w.blo = np.array([-0.5], np.float32); w.bhi = np.array([0.5], np.float32)
+    o = Oracle(w)
+    x0 = np.array([0.0, 0.2, 0.0, 0.0], np.float32)
+    r = o.step(x0, np.array([0.0], np.float32), 0, detail=True)
+    rho64 = float(np.float32(rho)); b = float(np.float32(0.1)); x1 = float(x0[1])
+    mixed = set()
+    for i in range(w.N + 1):
+        u = float(r["U"][i, 0])
+        expect = w.H
+        for k in range(1, w.H + 1):
+            xk = rho64 ** k * x1 + (1 - rho64 ** k) / (1 - rho64) * b * u
+            if not (-0.5 < xk < 0.5):
+                expect = k - 1
+                break
+        assert r["steps_all"][i] == expect
+        mixed.add(expect == w.H)
+    assert mixed == {True, False}
+
+
+def test_special_case_B_zero():
+    """B = 0: all candidates share one trajectory => all safe (nearest sample wins) or all unsafe
+    with equal steps (index 0 wins)."""
+    w = W.make("C1", N=64, H=20)
+    w.B = np.zeros_like(w.B)
+    o = Oracle(w)
+    r = o.step(w.x_nom, np.array([0.123], np.float32), 5, detail=True)
+    assert r["n_safe"] == w.N + 1 and r["index"] == w.N and r["dist"] == 0
+    o0 = Oracle(w, include_user=0)
+    r0 = o0.step(w.x_nom, np.array([0.123], np.float32), 5, detail=True)
+    assert r0["index"] == int(np.argmin(np.abs(r0["U"][:, 0].astype(np.float64) - np.float64(np.float32(0.123)))))
+    bad = np.array([1.9, 0.49, 3.0, 3.0], np.float32)                   # leaves the box under K alone
+    rb = o.step(bad, np.array([0.123], np.float32), 5, detail=True)
+    if rb["safe"] == 0:
+        assert rb["index"] == 0 and len(set(rb["steps_all"])) == 1
+
+
+# ---------------------------------------------------------------- P7: structural invariants ------
+def test_prefix_and_monotone_invariants():
+    w = W.make("C2", N=400)
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        full = Oracle(w).step(x0, uu, int(t), detail=True)
+        for Hp in (1, 17, 60):
+            part = Oracle(w, H=Hp).step(x0, uu, int(t), detail=True)
+            assert np.array_equal(part["steps_all"], np.minimum(full["steps_all"], Hp))   # prefix
+        big = Oracle(G.scaled_bounds(w, 1.5)).step(x0, uu, int(t), detail=True)
+        assert np.all(big["steps_all"] >= full["steps_all"])                               # monotone
+        if full["safe"]:
+            assert big["safe"] and big["dist"] <= full["dist"]
+        # inflated barrier shrinks the safe set
+        import copy
+        wi = copy.copy(w); wi.inflate = 0.05
+        infl = Oracle(wi).step(x0, uu, int(t), detail=True)
+        assert np.all(infl["steps_all"] <= full["steps_all"])
+
+
+def test_is_safe_conventions():
+    """box strict, annulus closed, NaN/Inf => unsafe (DESIGN G9)."""
+    w = W.make("C1")
+    o = Oracle(w)
+    assert o.is_safe([0, 0, 0, 0])[0] and not o.is_safe([2.0, 0, 0, 0])[0] and not o.is_safe([0, -0.5, 0, 0])[0]
+    assert not o.is_safe([np.nan, 0, 0, 0])[0] and not o.is_safe([0, np.inf, 0, 0])[0]
+    assert abs(o.is_safe([1.5, 0.1, 9, 9])[1] - 0.4) < 1e-12
+    w3 = W.make("C3")
+    o3 = Oracle(w3)
+    assert o3.is_safe([8, 0, 0, 0, 0, 0])[0] and o3.is_safe([0, -12, 0, 0, 0, 0])[0]
+    assert not o3.is_safe([7.999, 0, 0, 0, 0, 0])[0] and not o3.is_safe([np.nan, 0, 0, 0, 0, 0])[0]
+    assert abs(o3.is_safe([3.0, 4.0 + 5, 0, 0, 0, 0])[1] - min(abs(np.hypot(3, 9) - 8), abs(12 - np.hypot(3, 9)))) < 1e-12
+
+
+def test_rollout_batch_matches_single():
+    w = W.make("C3", N=32)
+    o = Oracle(w)
+    rng = np.random.default_rng(1)
+    U = rng.uniform(-1, 1, (32, 2)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, 32)
+    steps, marg, traj = o.rollout_batch(U, x0s, want_traj=True)
+    for i in (0, 7, 31):
+        s, mg, tr = o.rollout(o.lift(x0s[i].astype(np.float64)), U[i].astype(np.float64), want_traj=True)
+        assert s == steps[i] and mg == marg[i] and np.array_equal(np.nan_to_num(tr), np.nan_to_num(traj[i]))
+        e = min(s + 1, w.H)
+        assert np.all(np.isfinite(traj[i, :e])) and np.all(np.isnan(traj[i, e:]))
+
+
+def test_calibrated_workloads_are_mixed():
+    """safe fraction at x_nom inside Table I's band."""
+    for name in ("C1", "C2", "C3", "C5"):
+        w = W.make(name, N=2048 if name != "C3" else 10000)
+        r = Oracle(w, include_user=0).step(w.x_nom, np.zeros(w.m, np.float32), 0)
+        assert 0.28 <= r["n_safe"] / w.N <= 0.50, (name, r["n_safe"] / w.N)
