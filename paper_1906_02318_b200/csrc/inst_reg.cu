@@ -1,0 +1,30 @@
+// inst_reg.cu -- instantiates the register-resident kernels for one (MPMI_D, MPMI_MODE); compiled
+// once per pair by build.py so that the translation units build in parallel.
+#include "rollout_reg.cuh"
+#ifndef MPMI_D
+#error "compile with -DMPMI_D=8|16|32 -DMPMI_MODE=0|1"
+#endif
+using namespace mpmi;
+#if MPMI_MODE == 0
+#define FN(D) mpmi_pick_reg_##D##_tick
+#else
+#define FN(D) mpmi_pick_reg_##D##_batch
+#endif
+#define FN2(D) FN(D)
+
+template <int M>
+static KernFn pick_p(int P) {
+    constexpr int PW = 32 / MPMI_D;                 // wide packing: 2*PW candidates per thread
+    if (P == 1) return rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE>;
+    if (P == PW) return rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE>;
+    return nullptr;
+}
+KernFn FN2(MPMI_D)(int M, int P) {
+    switch (M) {
+        case 1: return pick_p<1>(P);
+        case 2: return pick_p<2>(P);
+        case 3: return pick_p<3>(P);
+        case 4: return pick_p<4>(P);
+    }
+    return nullptr;
+}

@@ -1,0 +1,36 @@
+// kernel_args.cuh -- launch-time argument block shared by the host runtime and the kernels.
+#pragma once
+#include "mpmi_device.cuh"
+
+namespace mpmi {
+
+constexpr int kRegBlock = 128;
+
+struct KArgs {
+    // tick
+    const float *x0;                      // device, n   (MODE_TICK; MODE_BATCH with x0_count == 1)
+    const float *u_user;                  // device, m
+    const unsigned long long *tick_ptr;   // device or null -> tick_val
+    unsigned long long tick_val;
+    TickState *st;
+    mpmi_result *out;
+    mpmi_partial *partial;
+    // batch
+    const float *U;                       // device Ncand*m or null
+    long long x0_count;
+    long long ncand;                      // candidates handled by this launch (local)
+    int H;
+    int dump_kind;
+    float *traj;
+    int *steps;
+    uint8_t *safe;
+};
+
+enum { MODE_TICK = 0, MODE_BATCH = 1 };
+
+constexpr int kTileThreads = 256;
+constexpr int kTileNC = 256;
+
+}  // namespace mpmi
+
+typedef void (*KernFn)(const mpmi::DevCfg, const mpmi::KArgs);

@@ -1,0 +1,430 @@
+// mpmi_api.cu -- host runtime and C ABI (include/mpmi.h) of the B200-native MPMI-SC tick.
+// Context creation (validation, internal re-ordering / padding of the model, upload), kernel
+// choice, the per-tick CUDA graph (param H2D -> fused tick kernel -> result D2H),
+// pinned staging, and the benchmark entry mpmi_rollout_batch.  No CPU fallback: every step of the
+// path runs in the kernels of rollout_reg.cuh / rollout_tile.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+#include <cuda_runtime.h>
+#include "../../include/mpmi.h"
+#include "mpmi_device.cuh"
+#include "kernel_args.cuh"
+
+using namespace mpmi;
+
+
+struct mpmi_ctx {
+    DevCfg dc;
+    int device = 0, sm_count = 0;
+    int variant = 0, P = 1, block = 128, cand_per_block = 0, smem = 0, regs = 0;
+    KernFn k_tick = nullptr, k_batch = nullptr;
+    float *d_KTa = nullptr, *d_W = nullptr, *d_b = nullptr;
+    uint8_t *d_terms = nullptr;
+    TickIn *d_in = nullptr, *h_in = nullptr;
+    TickState *d_state = nullptr;
+    mpmi_result *d_res = nullptr, *h_res = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaEvent_t done = nullptr;
+    bool pending = false;
+    std::string err;
+};
+
+namespace mpmi {
+// a7 for the sharded path: reduce G partials and decode.
+__global__ void shard_finalise_kernel(const __grid_constant__ DevCfg cfg, const mpmi_partial *parts, int G,
+                                      const float *u_user, unsigned long long tick, mpmi_result *out) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    unsigned long long k = kKeyNone, ne = 0; unsigned ns = 0;
+    for (int g = 0; g < G; g++) {
+        k = parts[g].key < k ? parts[g].key : k;
+        ns += (unsigned)parts[g].n_safe; ne += (unsigned long long)parts[g].n_exec;
+    }
+    float u_h[kMaxM];
+    clamp_user(cfg, u_user, u_h);
+    decode_result(cfg, k, ne, ns, tick, u_h, out);
+}
+
+}  // namespace mpmi
+
+namespace {
+
+thread_local std::string g_create_err;
+
+#define CU(ctx, call)                                                                      \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess) {                                                           \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);               \
+            return e_ == cudaErrorMemoryAllocation ? MPMI_ERR_NOMEM : MPMI_ERR_CUDA;       \
+        }                                                                                  \
+    } while (0)
+
+int fail(mpmi_ctx *c, int code, const char *msg) {
+    if (c) c->err = msg;
+    g_create_err = msg;
+    return code;
+}
+
+// kernel tables live in inst_reg.cu / inst_tile.cu, one translation unit per (D, MODE)
+#define MPMI_DECL_REG(D) KernFn mpmi_pick_reg_##D##_tick(int M, int P); KernFn mpmi_pick_reg_##D##_batch(int M, int P);
+#define MPMI_DECL_TILE(D) KernFn mpmi_pick_tile_##D##_tick(int M, int *smem); KernFn mpmi_pick_tile_##D##_batch(int M, int *smem);
+}  // namespace
+MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
+namespace {
+KernFn pick_reg(int D, int M, int P, int mode) {
+    const bool t = mode == MODE_TICK;
+    switch (D) {
+        case 8: return t ? mpmi_pick_reg_8_tick(M, P) : mpmi_pick_reg_8_batch(M, P);
+        case 16: return t ? mpmi_pick_reg_16_tick(M, P) : mpmi_pick_reg_16_batch(M, P);
+        case 32: return t ? mpmi_pick_reg_32_tick(M, P) : mpmi_pick_reg_32_batch(M, P);
+    }
+    return nullptr;
+}
+KernFn pick_tile(int D, int M, int mode, int *smem) {
+    const bool t = mode == MODE_TICK;
+    if (D == 64) return t ? mpmi_pick_tile_64_tick(M, smem) : mpmi_pick_tile_64_batch(M, smem);
+    if (D == 128) return t ? mpmi_pick_tile_128_tick(M, smem) : mpmi_pick_tile_128_batch(M, smem);
+    return nullptr;
+}
+
+bool all_finite(const float *p, size_t n) {
+    for (size_t i = 0; i < n; i++) if (!std::isfinite(p[i])) return false;
+    return true;
+}
+
+void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a, cudaStream_t s) {
+    long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
+    if (blocks < 1) blocks = 1;
+    void *args[2] = {(void *)&c->dc, (void *)&a};
+    cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)c->block), args, (size_t)c->smem, s);
+}
+
+int build_graph(mpmi_ctx *c) {
+    cudaStream_t s;
+    CU(c, cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+    KArgs a{};
+    a.x0 = c->d_in->x0; a.u_user = c->d_in->u_user; a.tick_ptr = &c->d_in->tick;
+    a.st = c->d_state; a.out = c->d_res;
+    CU(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+    cudaMemcpyAsync(c->d_in, c->h_in, sizeof(TickIn), cudaMemcpyHostToDevice, s);
+    launch(c, c->k_tick, c->dc.shard_count, a, s);
+    cudaMemcpyAsync(c->h_res, c->d_res, sizeof(mpmi_result), cudaMemcpyDeviceToHost, s);
+    CU(c, cudaStreamEndCapture(s, &c->graph));
+    CU(c, cudaGraphInstantiate(&c->exec, c->graph, 0));
+    CU(c, cudaStreamDestroy(s));
+    return MPMI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *mpmi_strerror(int status) {
+    switch (status) {
+        case MPMI_OK: return "ok";
+        case MPMI_ERR_INVALID: return "invalid argument";
+        case MPMI_ERR_UNSUPPORTED: return "unsupported configuration or device";
+        case MPMI_ERR_CUDA: return "CUDA runtime error";
+        case MPMI_ERR_NOMEM: return "out of memory";
+    }
+    return "unknown status";
+}
+
+const char *mpmi_last_error(const mpmi_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+void mpmi_destroy(mpmi_ctx *c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    if (c->done) { cudaEventSynchronize(c->done); cudaEventDestroy(c->done); }
+    if (c->exec) cudaGraphExecDestroy(c->exec);
+    if (c->graph) cudaGraphDestroy(c->graph);
+    cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
+    cudaFree(c->d_in); cudaFree(c->d_state); cudaFree(c->d_res);
+    cudaFreeHost(c->h_in); cudaFreeHost(c->h_res);
+    delete c;
+}
+
+int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
+    g_create_err.clear();
+    if (!cfg || !out) return fail(nullptr, MPMI_ERR_INVALID, "null config or output pointer");
+    *out = nullptr;
+    const int n = cfg->n, m = cfg->m, d = cfg->d;
+    if (n <= 0 || m <= 0 || d <= 0 || cfg->N <= 0 || cfg->H <= 0) return fail(nullptr, MPMI_ERR_INVALID, "n, m, d, N, H must be positive");
+    if (m > MPMI_MAX_M || n > MPMI_MAX_N || d > MPMI_MAX_D) return fail(nullptr, MPMI_ERR_UNSUPPORTED, "m > 4, n > 16 or d > 128");
+    if (n > d) return fail(nullptr, MPMI_ERR_INVALID, "n > d: the first n lifted features must be the state");
+    if (cfg->N > MPMI_MAX_CAND || cfg->H > 65535) return fail(nullptr, MPMI_ERR_UNSUPPORTED, "N or H too large");
+    if (!cfg->K || !cfg->B || !cfg->u_lo || !cfg->u_hi) return fail(nullptr, MPMI_ERR_INVALID, "null K, B, u_lo or u_hi");
+    if (!all_finite(cfg->K, (size_t)d * d) || !all_finite(cfg->B, (size_t)d * m)) return fail(nullptr, MPMI_ERR_INVALID, "non-finite K or B");
+    if (!all_finite(cfg->u_lo, m) || !all_finite(cfg->u_hi, m)) return fail(nullptr, MPMI_ERR_INVALID, "non-finite input box");
+    for (int j = 0; j < m; j++) if (cfg->u_lo[j] > cfg->u_hi[j]) return fail(nullptr, MPMI_ERR_INVALID, "u_lo > u_hi");
+    if (cfg->sampler != MPMI_SAMPLER_PHILOX && cfg->sampler != MPMI_SAMPLER_GRID) return fail(nullptr, MPMI_ERR_INVALID, "unknown sampler");
+    if (cfg->sampler == MPMI_SAMPLER_GRID) {
+        if (!cfg->grid_counts) return fail(nullptr, MPMI_ERR_INVALID, "grid sampler without grid_counts");
+        long long prod = 1;
+        for (int j = 0; j < m; j++) {
+            if (cfg->grid_counts[j] <= 0) return fail(nullptr, MPMI_ERR_INVALID, "grid count <= 0");
+            prod *= cfg->grid_counts[j];
+            if (prod > MPMI_MAX_CAND) break;
+        }
+        if (prod != cfg->N) return fail(nullptr, MPMI_ERR_INVALID, "N != product of grid_counts");
+    }
+    const mpmi_lift_spec &L = cfg->lift;
+    if (L.kind == MPMI_LIFT_MONO) {
+        if (!L.terms) return fail(nullptr, MPMI_ERR_INVALID, "MONO lift without terms");
+        for (int f = 0; f < d; f++)
+            for (int q = 0; q < 4; q++) {
+                const unsigned code = L.terms[4 * f + q];
+                if (code != 0xFF && ((code >> 6) > 2 || (int)(code & 0x3F) >= n)) return fail(nullptr, MPMI_ERR_INVALID, "bad lift factor code");
+            }
+        for (int j = 0; j < n; j++)
+            if (L.terms[4 * j] != j || L.terms[4 * j + 1] != 0xFF || L.terms[4 * j + 2] != 0xFF || L.terms[4 * j + 3] != 0xFF)
+                return fail(nullptr, MPMI_ERR_INVALID, "the first n lift features must be the state itself");
+    } else if (L.kind == MPMI_LIFT_RFF) {
+        if (d > n && (!L.W || !L.b)) return fail(nullptr, MPMI_ERR_INVALID, "RFF lift without W or b");
+        if (d > n && (!all_finite(L.W, (size_t)(d - n) * n) || !all_finite(L.b, d - n) || !std::isfinite(L.scale)))
+            return fail(nullptr, MPMI_ERR_INVALID, "non-finite RFF table");
+    } else {
+        return fail(nullptr, MPMI_ERR_INVALID, "unknown lift kind");
+    }
+    const mpmi_safe_spec &S = cfg->safe;
+    if (S.nbounds < 0 || S.nbounds > MPMI_MAX_BOUNDS || (S.nbounds > 0 && (!S.idx || !S.lo || !S.hi))) return fail(nullptr, MPMI_ERR_INVALID, "bad box constraints");
+    for (int q = 0; q < S.nbounds; q++) {
+        if (S.idx[q] < 0 || S.idx[q] >= n) return fail(nullptr, MPMI_ERR_INVALID, "box constraint index >= n");
+        if (std::isnan(S.lo[q]) || std::isnan(S.hi[q])) return fail(nullptr, MPMI_ERR_INVALID, "NaN box limit");
+    }
+    if (!std::isfinite(S.inflate)) return fail(nullptr, MPMI_ERR_INVALID, "non-finite inflate");
+    if (S.annulus) {
+        if (S.ix < 0 || S.ix >= n || S.iy < 0 || S.iy >= n || S.ix == S.iy) return fail(nullptr, MPMI_ERR_INVALID, "bad annulus coordinates");
+        if (!std::isfinite(S.cx) || !std::isfinite(S.cy) || !std::isfinite(S.rmin) || !std::isfinite(S.rmax) || S.rmin < 0)
+            return fail(nullptr, MPMI_ERR_INVALID, "bad annulus radii");
+    }
+    const long long ncg = (long long)cfg->N + (cfg->include_user ? 1 : 0);
+    long long sb = cfg->shard_begin, sc = cfg->shard_count;
+    if (sb == 0 && sc == 0) sc = ncg;
+    if (sb < 0 || sc <= 0 || sb + sc > ncg) return fail(nullptr, MPMI_ERR_INVALID, "shard outside [0, N + include_user]");
+
+    int dev = cfg->device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return fail(nullptr, MPMI_ERR_CUDA, "no CUDA device");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(nullptr, MPMI_ERR_CUDA, "cudaGetDeviceProperties failed");
+    if (prop.major != 10) return fail(nullptr, MPMI_ERR_UNSUPPORTED, "device is not compute capability 10.x (kernels are sm_100a only)");
+
+    mpmi_ctx *c = new (std::nothrow) mpmi_ctx();
+    if (!c) return fail(nullptr, MPMI_ERR_NOMEM, "host allocation failed");
+    c->device = dev;
+    c->sm_count = prop.multiProcessorCount;
+    int rc = MPMI_OK;
+    auto bail = [&](int code) { g_create_err = c->err; mpmi_destroy(c); return code; };
+    if (cudaSetDevice(dev) != cudaSuccess) { c->err = "cudaSetDevice failed"; return bail(MPMI_ERR_CUDA); }
+
+    // ---- internal ordering of the physical dims: annulus coordinates, then box dims, then the rest
+    DevCfg &dc = c->dc;
+    std::memset(&dc, 0, sizeof dc);
+    std::vector<int> perm;
+    std::vector<char> used(n, 0);
+    if (S.annulus) { perm.push_back(S.ix); perm.push_back(S.iy); used[S.ix] = used[S.iy] = 1; }
+    for (int j = 0; j < n; j++) {
+        bool boxed = false;
+        for (int q = 0; q < S.nbounds; q++) boxed = boxed || S.idx[q] == j;
+        if (boxed && !used[j]) { perm.push_back(j); used[j] = 1; }
+    }
+    for (int j = 0; j < n; j++) if (!used[j]) perm.push_back(j);
+    auto po = [&](int f) { return f < n ? perm[f] : f; };
+
+    const int D = d <= 8 ? 8 : d <= 16 ? 16 : d <= 32 ? 32 : d <= 64 ? 64 : 128;
+    dc.n = n; dc.m = m; dc.d = d; dc.D = D;
+    dc.N = cfg->N; dc.H = cfg->H; dc.include_user = cfg->include_user ? 1 : 0;
+    dc.ncand_global = ncg; dc.shard_begin = sb; dc.shard_count = sc;
+    dc.sampler = cfg->sampler;
+    dc.seed_lo = (unsigned)cfg->seed; dc.seed_hi = (unsigned)(cfg->seed >> 32);
+    for (int j = 0; j < kMaxM; j++) {
+        dc.grid_counts[j] = (cfg->sampler == MPMI_SAMPLER_GRID && j < m) ? cfg->grid_counts[j] : 1;
+        dc.u_lo[j] = j < m ? cfg->u_lo[j] : 0.f;
+        dc.u_hi[j] = j < m ? cfg->u_hi[j] : 0.f;
+    }
+    dc.lift_kind = L.kind; dc.rff_scale = L.scale;
+    for (int j = 0; j < kMaxN; j++) { dc.blo[j] = -INFINITY; dc.bhi[j] = INFINITY; dc.perm[j] = (unsigned char)(j < n ? perm[j] : j); }
+    for (int q = 0; q < S.nbounds; q++) {
+        int ji = 0;
+        while (perm[ji] != S.idx[q]) ji++;
+        const float lo = (float)((double)S.lo[q] + (double)S.inflate), hi = (float)((double)S.hi[q] - (double)S.inflate);
+        dc.blo[ji] = std::fmax(dc.blo[ji], lo);
+        dc.bhi[ji] = std::fmin(dc.bhi[ji], hi);
+        dc.bmask |= 1u << ji;
+    }
+    dc.annulus = S.annulus ? 1 : 0;
+    if (S.annulus) {
+        const double rmin = (double)S.rmin + S.inflate, rmax = (double)S.rmax - S.inflate;
+        dc.cx = S.cx; dc.cy = S.cy;
+        dc.rmin2 = (float)(rmin * rmin); dc.rmax2 = rmax < 0 ? -1.f : (float)(rmax * rmax);
+    }
+
+    // ---- augmented transposed model KTa[c][r]: c < D -> K[r][c], c >= D -> B[r][c-D]; zero padded
+    const int M = m;
+    std::vector<float> KTa((size_t)(D + M) * D, 0.f);
+    for (int r = 0; r < d; r++) {
+        for (int q = 0; q < d; q++) KTa[(size_t)q * D + r] = cfg->K[(size_t)po(r) * d + po(q)];
+        for (int j = 0; j < m; j++) KTa[(size_t)(D + j) * D + r] = cfg->B[(size_t)po(r) * m + j];
+    }
+    std::vector<uint8_t> terms((size_t)D * 4, 0xFF);
+    if (L.kind == MPMI_LIFT_MONO)
+        for (int f = 0; f < d; f++) std::memcpy(&terms[4 * f], &L.terms[4 * po(f)], 4);
+
+#define CUC(call) do { rc = [&]() -> int { CU(c, call); return MPMI_OK; }(); if (rc != MPMI_OK) return bail(rc); } while (0)
+    CUC(cudaMalloc(&c->d_KTa, KTa.size() * sizeof(float)));
+    CUC(cudaMemcpy(c->d_KTa, KTa.data(), KTa.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUC(cudaMalloc(&c->d_terms, terms.size()));
+    CUC(cudaMemcpy(c->d_terms, terms.data(), terms.size(), cudaMemcpyHostToDevice));
+    if (L.kind == MPMI_LIFT_RFF && d > n) {
+        CUC(cudaMalloc(&c->d_W, (size_t)(d - n) * n * sizeof(float)));
+        CUC(cudaMemcpy(c->d_W, L.W, (size_t)(d - n) * n * sizeof(float), cudaMemcpyHostToDevice));
+        CUC(cudaMalloc(&c->d_b, (size_t)(d - n) * sizeof(float)));
+        CUC(cudaMemcpy(c->d_b, L.b, (size_t)(d - n) * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    dc.KTa = c->d_KTa; dc.terms = c->d_terms; dc.W = c->d_W; dc.b = c->d_b;
+    CUC(cudaMalloc(&c->d_in, sizeof(TickIn)));
+    CUC(cudaMemset(c->d_in, 0, sizeof(TickIn)));
+    CUC(cudaMalloc(&c->d_state, sizeof(TickState)));
+    TickState st0{kKeyNone, 0ull, 0u, 0u};
+    CUC(cudaMemcpy(c->d_state, &st0, sizeof st0, cudaMemcpyHostToDevice));
+    CUC(cudaMalloc(&c->d_res, sizeof(mpmi_result)));
+    CUC(cudaHostAlloc(&c->h_in, sizeof(TickIn), cudaHostAllocDefault));
+    CUC(cudaHostAlloc(&c->h_res, sizeof(mpmi_result), cudaHostAllocDefault));
+    std::memset(c->h_in, 0, sizeof(TickIn));
+    CUC(cudaEventCreateWithFlags(&c->done, cudaEventDisableTiming));
+
+    // ---- kernel choice ------------------------------------------------------------------------------
+    if (D <= 32) {
+        c->variant = 1;
+        const int Pmax = 32 / D;
+        // enough warps to give every SM sub-partition two warps at the wide packing?  else 2 cand/thread
+        const long long warps_wide = (sc + 2LL * Pmax * 32 - 1) / (2LL * Pmax * 32);
+        c->P = (cfg->variant == 11) ? 1 : (cfg->variant == 12) ? Pmax : (warps_wide >= 8LL * c->sm_count ? Pmax : 1);
+        const long long threads = (sc + 2LL * c->P - 1) / (2LL * c->P);
+        c->block = threads >= 128LL * 2 * c->sm_count ? 128 : threads >= 64LL * 2 * c->sm_count ? 64 : 32;
+        c->cand_per_block = 2 * c->P * c->block;
+        c->smem = 0;
+        c->k_tick = pick_reg(D, M, c->P, MODE_TICK);
+        c->k_batch = pick_reg(D, M, c->P, MODE_BATCH);
+    } else {
+        c->variant = 2;
+        c->P = 1; c->block = kTileThreads; c->cand_per_block = kTileNC;
+        c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem);
+        c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem);
+        if (c->k_tick) {
+            CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
+            CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
+        }
+    }
+    if (!c->k_tick || !c->k_batch) { c->err = "no kernel for this (d, m)"; return bail(MPMI_ERR_UNSUPPORTED); }
+    cudaFuncAttributes fa;
+    CUC(cudaFuncGetAttributes(&fa, (const void *)c->k_tick));
+    c->regs = fa.numRegs;
+    rc = build_graph(c);
+    if (rc != MPMI_OK) return bail(rc);
+#undef CUC
+    *out = c;
+    return MPMI_OK;
+}
+
+int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
+    if (!c || !o) return MPMI_ERR_INVALID;
+    std::memset(o, 0, sizeof *o);
+    o->d_pad = c->dc.D; o->variant = c->variant; o->cand_per_block = c->cand_per_block;
+    o->threads_per_block = c->block;
+    o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
+    o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
+    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = 1; o->uses_graph = 1;
+    o->ncand_local = c->dc.shard_count;
+    return MPMI_OK;
+}
+
+int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, void *stream) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (!x0 || !u_user) return fail(c, MPMI_ERR_INVALID, "null x0 or u_user");
+    if (!all_finite(x0, c->dc.n) || !all_finite(u_user, c->dc.m)) return fail(c, MPMI_ERR_INVALID, "non-finite x0 or u_user");
+    CU(c, cudaSetDevice(c->device));
+    if (c->pending) { CU(c, cudaEventSynchronize(c->done)); c->pending = false; }   // one tick in flight
+    std::memcpy(c->h_in->x0, x0, sizeof(float) * c->dc.n);
+    std::memcpy(c->h_in->u_user, u_user, sizeof(float) * c->dc.m);
+    c->h_in->tick = tick;
+    CU(c, cudaGraphLaunch(c->exec, (cudaStream_t)stream));
+    CU(c, cudaEventRecord(c->done, (cudaStream_t)stream));
+    c->pending = true;
+    c->err.clear();
+    return MPMI_OK;
+}
+
+int mpmi_step_result(mpmi_ctx *c, mpmi_result *out) {
+    if (!c || !out) return MPMI_ERR_INVALID;
+    if (!c->pending) return fail(c, MPMI_ERR_INVALID, "no tick in flight");
+    CU(c, cudaEventSynchronize(c->done));
+    c->pending = false;
+    *out = *c->h_res;
+    return MPMI_OK;
+}
+
+int mpmi_step_sync(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, void *stream, mpmi_result *out) {
+    if (!out) return MPMI_ERR_INVALID;
+    const int rc = mpmi_step(c, x0, u_user, tick, stream);
+    return rc != MPMI_OK ? rc : mpmi_step_result(c, out);
+}
+
+int mpmi_step_device(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint64_t tick, void *stream, mpmi_result *d_out) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (!d_x0 || !d_u_user || !d_out) return fail(c, MPMI_ERR_INVALID, "null device pointer");
+    CU(c, cudaSetDevice(c->device));
+    KArgs a{};
+    a.x0 = d_x0; a.u_user = d_u_user; a.tick_ptr = nullptr; a.tick_val = tick;
+    a.st = c->d_state; a.out = d_out;
+    launch(c, c->k_tick, c->dc.shard_count, a, (cudaStream_t)stream);
+    CU(c, cudaGetLastError());
+    return MPMI_OK;
+}
+
+int mpmi_shard_step(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint64_t tick, void *stream, mpmi_partial *d_partial) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (!d_x0 || !d_u_user || !d_partial) return fail(c, MPMI_ERR_INVALID, "null device pointer");
+    CU(c, cudaSetDevice(c->device));
+    KArgs a{};
+    a.x0 = d_x0; a.u_user = d_u_user; a.tick_ptr = nullptr; a.tick_val = tick;
+    a.st = c->d_state; a.out = nullptr; a.partial = d_partial;
+    launch(c, c->k_tick, c->dc.shard_count, a, (cudaStream_t)stream);
+    CU(c, cudaGetLastError());
+    return MPMI_OK;
+}
+
+int mpmi_shard_finalize(mpmi_ctx *c, const mpmi_partial *d_partials, int32_t G, const float *d_u_user, uint64_t tick,
+                        void *stream, mpmi_result *d_out) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (!d_partials || G <= 0 || !d_u_user || !d_out) return fail(c, MPMI_ERR_INVALID, "bad shard_finalize arguments");
+    CU(c, cudaSetDevice(c->device));
+    shard_finalise_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(c->dc, d_partials, G, d_u_user, tick, d_out);
+    CU(c, cudaGetLastError());
+    return MPMI_OK;
+}
+
+int mpmi_rollout_batch(mpmi_ctx *c, const float *d_U, const float *d_X0, int64_t x0_count, int64_t Ncand, int32_t H,
+                       int32_t dump_kind, float *d_traj, int32_t *d_steps, uint8_t *d_safe, uint64_t tick, void *stream) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (!d_X0 || !d_steps) return fail(c, MPMI_ERR_INVALID, "null d_X0 or d_steps");
+    if (Ncand <= 0 || Ncand > MPMI_MAX_CAND || H <= 0 || H > 65535) return fail(c, MPMI_ERR_INVALID, "bad Ncand or H");
+    if (x0_count != 1 && x0_count != Ncand) return fail(c, MPMI_ERR_INVALID, "x0_count must be 1 or Ncand");
+    if (dump_kind < MPMI_DUMP_NONE || dump_kind > MPMI_DUMP_LIFTED || (dump_kind != MPMI_DUMP_NONE && !d_traj))
+        return fail(c, MPMI_ERR_INVALID, "bad dump_kind or null d_traj");
+    CU(c, cudaSetDevice(c->device));
+    KArgs a{};
+    a.x0 = d_X0; a.u_user = nullptr; a.tick_ptr = nullptr; a.tick_val = tick;
+    a.U = d_U; a.x0_count = x0_count; a.ncand = Ncand; a.H = H; a.dump_kind = dump_kind;
+    a.traj = d_traj; a.steps = d_steps; a.safe = d_safe;
+    launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream);
+    CU(c, cudaGetLastError());
+    return MPMI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,269 @@
+// mpmi_device.cuh -- device-side building blocks of the MPMI-SC tick (Algorithm 2):
+// sampler (a1), lift (a2), safe test (a4), selection key (a5), reductions (a6), finalise (a7).
+// sm_100a only.  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/mpmi.h"
+
+namespace mpmi {
+
+constexpr int kMaxM = MPMI_MAX_M;
+constexpr int kMaxN = MPMI_MAX_N;
+
+// Everything the kernels need, passed by value as a __grid_constant__ kernel parameter so that
+// bounds, box limits and sampler constants are direct constant-bank operands.
+struct DevCfg {
+    int n, m, d, D;                 // D = padded lifted dim (zero rows / columns)
+    int N, H, include_user;
+    long long ncand_global;         // N + include_user
+    long long shard_begin, shard_count;
+    int sampler;
+    int grid_counts[kMaxM];
+    unsigned seed_lo, seed_hi;
+    float u_lo[kMaxM], u_hi[kMaxM];
+    int lift_kind;
+    float rff_scale;
+    unsigned bmask;                 // bit j set: internal physical dim j has a box constraint
+    float blo[kMaxN], bhi[kMaxN];   // per INTERNAL dimension limits, inflation folded in (+-inf if none)
+    int annulus;                    // annulus on INTERNAL dims 0,1
+    float cx, cy, rmin2, rmax2;     // inflation folded in, squared
+    unsigned char perm[kMaxN];      // internal physical dim j = original dim perm[j] (annulus / box dims first)
+    const float *KTa;               // device: augmented transposed model, layout per variant
+    const float *Kpad;              // device: D*D row-major padded K (tile variant)
+    const float *Bpad;              // device: D*4 row-major padded B
+    const uint8_t *terms;           // device: D*4 lift factor codes (MONO)
+    const float *W, *b;             // device: RFF tables
+};
+
+// Inputs of one tick as they sit in device memory.
+struct TickIn {
+    float x0[kMaxN];
+    float u_user[kMaxM];
+    unsigned long long tick;
+    unsigned long long pad;
+};
+
+// Cross-block selection state; reset by the block that finalises the tick.
+struct TickState {
+    unsigned long long best_key;
+    unsigned long long n_exec;
+    unsigned int n_safe;
+    unsigned int ticket;
+};
+
+constexpr unsigned long long kKeyNone = 0x7FFFFFFFFFFFFFFFull;
+constexpr int kKeyIndexBits = 30;
+
+// ---- a1: Philox4x32-10 (Salmon et al. SC'11), counter-based; DESIGN G4 ------------------------
+__device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3,
+                                              unsigned k0, unsigned k1, unsigned (&out)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const unsigned n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// candidate input u_i for GLOBAL index gi.  gi == N is the injected u_h.
+__device__ __forceinline__ void sample_u(const DevCfg &cfg, long long gi, unsigned long long tick,
+                                         const float (&u_h)[kMaxM], float (&u)[kMaxM]) {
+#pragma unroll
+    for (int j = 0; j < kMaxM; j++) u[j] = 0.0f;
+    if (gi >= cfg.N) {
+#pragma unroll
+        for (int j = 0; j < kMaxM; j++) u[j] = u_h[j];
+        return;
+    }
+    if (cfg.sampler == MPMI_SAMPLER_PHILOX) {
+        unsigned w[4];
+        philox4x32_10((unsigned)gi, (unsigned)((unsigned long long)gi >> 32), (unsigned)tick,
+                      (unsigned)(tick >> 32), cfg.seed_lo, cfg.seed_hi, w);
+#pragma unroll
+        for (int j = 0; j < kMaxM; j++) {
+            if (j < cfg.m) {
+                const float r = __uint2float_rn(w[j] >> 8) * 0x1p-24f;       // exact
+                u[j] = __fmaf_rn(r, __fsub_rn(cfg.u_hi[j], cfg.u_lo[j]), cfg.u_lo[j]);
+            }
+        }
+    } else {
+        long long rem = gi;                                                    // row-major, dim 0 slowest
+#pragma unroll
+        for (int j = kMaxM - 1; j >= 0; j--) {
+            if (j < cfg.m) {
+                const int cnt = cfg.grid_counts[j];
+                const int k = (int)(rem % cnt);
+                rem /= cnt;
+                const float lo = cfg.u_lo[j], hi = cfg.u_hi[j];
+                float v;
+                if (cnt == 1)          v = __fmul_rn(0.5f, __fadd_rn(lo, hi));
+                else if (k == cnt - 1) v = hi;
+                else                   v = __fmaf_rn(__fdiv_rn((float)k, (float)(cnt - 1)), __fsub_rn(hi, lo), lo);
+                u[j] = v;
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void clamp_user(const DevCfg &cfg, const float *u_user, float (&u_h)[kMaxM]) {
+#pragma unroll
+    for (int j = 0; j < kMaxM; j++) {
+        float v = 0.0f;
+        if (j < cfg.m) {
+            v = u_user[j];
+            v = v < cfg.u_lo[j] ? cfg.u_lo[j] : v;
+            v = v > cfg.u_hi[j] ? cfg.u_hi[j] : v;
+        }
+        u_h[j] = v;
+    }
+}
+
+// ---- a2: lift, one feature.  Accurate sinf/cosf (no fast-math). ------------
+__device__ __forceinline__ float lift_factor(unsigned code, const float *x) {
+    if (code == 0xFFu) return 1.0f;
+    const float v = x[code & 0x3Fu];
+    const unsigned kind = code >> 6;
+    return kind == 0 ? v : (kind == 1 ? sinf(v) : cosf(v));
+}
+__device__ __forceinline__ float lift_feature(const DevCfg &cfg, int f, const float *x) {
+    // f is the INTERNAL feature index; x is the state in the caller's order
+    if (f >= cfg.d) return 0.0f;                       // zero padding
+    if (f < cfg.n) return x[cfg.perm[f]];
+    if (cfg.lift_kind == MPMI_LIFT_MONO) {
+        const uint8_t *t = cfg.terms + 4 * f;
+        float p = lift_factor(t[0], x);
+        p = __fmul_rn(p, lift_factor(t[1], x));
+        p = __fmul_rn(p, lift_factor(t[2], x));
+        p = __fmul_rn(p, lift_factor(t[3], x));
+        return p;
+    }
+    const int r = f - cfg.n;
+    float s = cfg.b[r];
+    for (int j = 0; j < cfg.n; j++) s = __fmaf_rn(cfg.W[r * cfg.n + j], x[j], s);
+    return __fmul_rn(cfg.rff_scale, cosf(s));
+}
+
+// ---- a5: selection key.  bit 63 = 0, bit 62 = unsafe, bits 61..30 = primary, bits 29..0 = index.
+// safe:   primary = bits of the fp32 squared distance (monotone for >= 0);
+// unsafe: primary = H - steps  (most safe steps first).  Lexicographic order == integer order.
+__device__ __forceinline__ unsigned long long make_key(bool safe, float dist2, int H, int steps, long long gi) {
+    const unsigned primary = safe ? __float_as_uint(dist2) : (unsigned)(H - steps);
+    return ((unsigned long long)(safe ? 0 : 1) << 62) | ((unsigned long long)primary << kKeyIndexBits) |
+           (unsigned long long)gi;
+}
+
+__device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int lane_mask) {
+    unsigned lo = (unsigned)v, hi = (unsigned)(v >> 32);
+    lo = __shfl_xor_sync(0xffffffffu, lo, lane_mask);
+    hi = __shfl_xor_sync(0xffffffffu, hi, lane_mask);
+    return ((unsigned long long)hi << 32) | lo;
+}
+__device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long w = shfl_xor_u64(v, o);
+        v = w < v ? w : v;
+    }
+    return v;
+}
+__device__ __forceinline__ unsigned warp_sum_u32(unsigned v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ---- a6 (block part) + a7: block min -> one 64-bit atomicMin per block; the last block to arrive
+// decodes the key, regenerates the winning input from its index and writes the result.
+// If `partial` is non-null the block writes the shard's mpmi_partial instead (multi-GPU path).
+__device__ __forceinline__ void decode_result(const DevCfg &cfg, unsigned long long key, unsigned long long n_exec,
+                                              unsigned n_safe, unsigned long long tick,
+                                              const float (&u_h)[kMaxM], mpmi_result *out) {
+    mpmi_result r;
+    const long long gi = (long long)(key & ((1ull << kKeyIndexBits) - 1));
+    const bool safe = ((key >> 62) & 1ull) == 0;
+    const unsigned primary = (unsigned)(key >> kKeyIndexBits);
+    float u[kMaxM];
+    sample_u(cfg, gi, tick, u_h, u);
+    float d2 = 0.0f;
+#pragma unroll
+    for (int j = 0; j < kMaxM; j++) {
+        r.u[j] = u[j];
+        const float df = __fsub_rn(u[j], u_h[j]);
+        d2 = __fmaf_rn(df, df, d2);
+    }
+    r.index = (int)gi;
+    r.safe = safe ? 1 : 0;
+    r.steps = safe ? cfg.H : cfg.H - (int)primary;
+    r.n_safe = (int)n_safe;
+    r.dist = sqrtf(d2);
+    r.reserved = 0;
+    r.n_exec = (long long)n_exec;
+    r.key = key;
+    if (key == kKeyNone) { r.index = -1; r.safe = 0; r.steps = 0; r.dist = 0.0f; }
+    *out = r;
+}
+
+template <int kWarps>
+__device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, unsigned long long key,
+                                                          unsigned n_safe, unsigned n_exec,
+                                                          unsigned long long tick, const float (&u_h)[kMaxM],
+                                                          TickState *st, mpmi_result *out, mpmi_partial *partial) {
+    __shared__ unsigned long long s_key[kWarps];
+    __shared__ unsigned s_safe[kWarps], s_exec[kWarps];
+    __shared__ bool s_last;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    key = warp_min_u64(key);
+    n_safe = warp_sum_u32(n_safe);
+    n_exec = warp_sum_u32(n_exec);
+    if (lane == 0) { s_key[warp] = key; s_safe[warp] = n_safe; s_exec[warp] = n_exec; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long k = s_key[0];
+        unsigned ns = s_safe[0];
+        unsigned long long ne = s_exec[0];
+#pragma unroll
+        for (int w = 1; w < kWarps; w++) {
+            if (w * 32 < (int)blockDim.x) { k = s_key[w] < k ? s_key[w] : k; ns += s_safe[w]; ne += s_exec[w]; }
+        }
+        atomicMin(&st->best_key, k);
+        if (ns) atomicAdd(&st->n_safe, ns);
+        atomicAdd(&st->n_exec, ne);
+        __threadfence();
+        const unsigned t = atomicAdd(&st->ticket, 1u);
+        s_last = (t == gridDim.x - 1);
+        if (s_last) {
+            __threadfence();
+            const unsigned long long bk = atomicMin(&st->best_key, kKeyNone);     // atomic read
+            const unsigned long long tot_exec = atomicAdd(&st->n_exec, 0ull);
+            const unsigned tot_safe = atomicAdd(&st->n_safe, 0u);
+            if (partial) {
+                partial->key = bk; partial->n_safe = tot_safe; partial->n_exec = (long long)tot_exec;
+            } else {
+                decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out);
+            }
+            st->best_key = kKeyNone; st->n_exec = 0ull; st->n_safe = 0u; st->ticket = 0u;   // ready for next tick
+            __threadfence();
+        }
+    }
+}
+
+__device__ __forceinline__ bool finite_inputs(const DevCfg &cfg, const float *x0, const float *u_user) {
+    bool ok = true;
+    for (int j = 0; j < cfg.n; j++) ok = ok && isfinite(x0[j]);
+    for (int j = 0; j < cfg.m; j++) ok = ok && isfinite(u_user[j]);
+    return ok;
+}
+
+__device__ __forceinline__ float4 lds128(unsigned addr) {
+    // volatile: keeps the compiler from hoisting the (loop-invariant) model loads out of the
+    // horizon loop, which would spill ~D*D registers
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+}  // namespace mpmi

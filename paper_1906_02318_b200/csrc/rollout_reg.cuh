@@ -1,0 +1,228 @@
+// rollout_reg.cuh -- register-resident rollout kernel for padded lifted dim D <= 32 (a1-a7, a9).
+//
+// Each thread owns 2P candidates; candidate pair p is packed into the two halves of float2
+// registers so that one FFMA2 (Blackwell packed fp32 FMA, fma.rn.f32x2) advances one row of two
+// candidates: a[p][r] += K[r][c] * z[p][c], the K value broadcast to both halves.  The model is
+// staged once per CTA in shared memory as the augmented transpose KTa[c][r] (c < D: K[r][c];
+// c >= D: B[r][c-D]) and read with warp-uniform LDS.128 (conflict-free broadcast); the candidate's
+// input u is appended to z as "state" D..D+M-1, so one step executes exactly D*(D+M) fp32 FMAs per
+// candidate -- the algorithmic count of z' = K z + B u.
+// The safe set is tested after every step; a warp leaves the horizon loop when none
+// of its candidates is alive.
+#pragma once
+#include "mpmi_device.cuh"
+#include "kernel_args.cuh"
+
+namespace mpmi {
+
+// box limits on internal dims 0..nbox-1 (strict), annulus on internal dims 0,1 (closed); NaN -> unsafe
+template <int NB>
+__device__ __forceinline__ bool safe_check(const DevCfg &cfg, const float (&x)[NB], int nbox) {
+    bool ok = true;
+    if (nbox > 0) {
+#pragma unroll
+        for (int j = 0; j < 2 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+        if (nbox > 2) {
+#pragma unroll
+            for (int j = 2; j < 4 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+            if (nbox > 4) {
+#pragma unroll
+                for (int j = 4; j < 8 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+                if (nbox > 8) {
+#pragma unroll
+                    for (int j = 8; j < 16 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+                }
+            }
+        }
+    }
+    if (cfg.annulus) {
+        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
+        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
+        ok = ok && (r2 >= cfg.rmin2) && (r2 <= cfg.rmax2);
+    }
+    return ok;
+}
+
+template <int D, int P>
+constexpr int reg_min_blocks() { return (D * P >= 32) ? 3 : 4; }
+
+template <int D, int M, int P, int MODE>
+__global__ void __launch_bounds__(kRegBlock, reg_min_blocks<D, P>())
+rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
+    constexpr int S = 2 * P;                 // candidates per thread
+    constexpr int NB = D < kMaxN ? D : kMaxN;
+    __shared__ __align__(16) float sK[(D + M) * D];
+    __shared__ float sz0[D];
+    __shared__ float sstage[MODE == MODE_BATCH ? D * kRegBlock : 1];
+
+    const int tid = threadIdx.x, bdim = blockDim.x;
+    for (int i = tid; i < (D + M) * D / 4; i += bdim)
+        reinterpret_cast<float4 *>(sK)[i] = reinterpret_cast<const float4 *>(cfg.KTa)[i];
+    const unsigned long long tick = a.tick_ptr ? *a.tick_ptr : a.tick_val;
+    const int H = (MODE == MODE_TICK) ? cfg.H : a.H;
+    const long long ncand = (MODE == MODE_TICK) ? cfg.shard_count : a.ncand;
+    const bool shared_x0 = (MODE == MODE_TICK) || a.x0_count == 1;
+
+    float u_h[kMaxM] = {0.f, 0.f, 0.f, 0.f};
+    bool inputs_ok = true;
+    if (MODE == MODE_TICK) {
+        inputs_ok = finite_inputs(cfg, a.x0, a.u_user);
+        clamp_user(cfg, a.u_user, u_h);
+    }
+    if (shared_x0) {
+        for (int f = tid; f < D; f += bdim) sz0[f] = lift_feature(cfg, f, a.x0);
+    }
+    __syncthreads();
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(sK);
+
+    // ---- a1 + a2: candidates of this thread ------------------------------------------------------
+    float2 z[P][D + M];
+    long long li[S];
+    bool alive[S];
+    int steps[S];
+#pragma unroll
+    for (int s = 0; s < S; s++) {
+        li[s] = (long long)blockIdx.x * (S * bdim) + s * bdim + tid;
+        const bool valid = li[s] < ncand && inputs_ok;
+        alive[s] = valid;
+        steps[s] = 0;
+        float u[kMaxM] = {0.f, 0.f, 0.f, 0.f};
+        if (li[s] < ncand) {
+            if (MODE == MODE_BATCH && a.U) {
+#pragma unroll
+                for (int j = 0; j < M; j++) u[j] = a.U[li[s] * cfg.m + (j < cfg.m ? j : 0)] * (j < cfg.m ? 1.f : 0.f);
+            } else {
+                sample_u(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li[s], tick, u_h, u);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < M; j++) {
+            if (s & 1) z[s >> 1][D + j].y = u[j]; else z[s >> 1][D + j].x = u[j];
+        }
+        if (shared_x0) {
+#pragma unroll
+            for (int c = 0; c < D; c++) {
+                if (s & 1) z[s >> 1][c].y = sz0[c]; else z[s >> 1][c].x = sz0[c];
+            }
+        } else {
+            // per-candidate x0 (benchmark entry only): lift through a private shared-memory column so
+            // that the lift code is not replicated D times
+            float x[kMaxN];
+            const long long row = li[s] < ncand ? li[s] : 0;
+            for (int j = 0; j < kMaxN; j++) x[j] = j < cfg.n ? a.x0[row * cfg.n + j] : 0.f;
+#pragma unroll 1
+            for (int c = 0; c < D; c++) sstage[c * kRegBlock + tid] = lift_feature(cfg, c, x);
+#pragma unroll
+            for (int c = 0; c < D; c++) {
+                const float v = sstage[c * kRegBlock + tid];
+                if (s & 1) z[s >> 1][c].y = v; else z[s >> 1][c].x = v;
+            }
+        }
+    }
+
+    // ---- a3 + a4: horizon loop --------------------------------------------------------------------
+    const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
+    const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
+    const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
+    int k = 0;
+    for (; k < H; k++) {
+        bool any = false;
+#pragma unroll
+        for (int s = 0; s < S; s++) any = any || alive[s];
+        if (!__any_sync(0xffffffffu, any)) break;
+
+        float2 acc[P][D];
+#pragma unroll
+        for (int c = 0; c < D + M; c++) {
+#pragma unroll
+            for (int r = 0; r < D; r += 4) {
+                const float4 kv = lds128(sbase + (c * D + r) * 4);
+#pragma unroll
+                for (int p = 0; p < P; p++) {
+                    const float2 zc = z[p][c];
+                    if (c == 0) {
+                        const float2 zero = make_float2(0.f, 0.f);
+                        acc[p][r + 0] = __ffma2_rn(make_float2(kv.x, kv.x), zc, zero);
+                        acc[p][r + 1] = __ffma2_rn(make_float2(kv.y, kv.y), zc, zero);
+                        acc[p][r + 2] = __ffma2_rn(make_float2(kv.z, kv.z), zc, zero);
+                        acc[p][r + 3] = __ffma2_rn(make_float2(kv.w, kv.w), zc, zero);
+                    } else {
+                        acc[p][r + 0] = __ffma2_rn(make_float2(kv.x, kv.x), zc, acc[p][r + 0]);
+                        acc[p][r + 1] = __ffma2_rn(make_float2(kv.y, kv.y), zc, acc[p][r + 1]);
+                        acc[p][r + 2] = __ffma2_rn(make_float2(kv.z, kv.z), zc, acc[p][r + 2]);
+                        acc[p][r + 3] = __ffma2_rn(make_float2(kv.w, kv.w), zc, acc[p][r + 3]);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < P; p++)
+#pragma unroll
+            for (int r = 0; r < D; r++) z[p][r] = acc[p][r];
+
+#pragma unroll
+        for (int s = 0; s < S; s++) {
+            float x[NB];
+#pragma unroll
+            for (int j = 0; j < NB; j++) x[j] = (s & 1) ? z[s >> 1][j].y : z[s >> 1][j].x;
+            const bool was_alive = alive[s];
+            const bool ok = safe_check<NB>(cfg, x, nbox);
+            alive[s] = was_alive && ok;
+            steps[s] += alive[s] ? 1 : 0;
+            if (dump && li[s] < ncand) {
+                // a9: traj[(k*J + j)*Ncand + i], candidate fastest -> a warp writes 128 contiguous bytes
+#pragma unroll
+                for (int j = 0; j < D; j++) {
+                    const int row = j < cfg.n ? (int)cfg.perm[j < kMaxN ? j : 0] : j;
+                    if (row < J) {
+                        const float v = (s & 1) ? z[s >> 1][j].y : z[s >> 1][j].x;
+                        a.traj[((long long)k * J + row) * ncand + li[s]] = was_alive ? v : __int_as_float(0x7fc00000);
+                    }
+                }
+            }
+        }
+    }
+    if (dump) {                              // states after the warp stopped: NaN
+        for (; k < H; k++)
+#pragma unroll
+            for (int s = 0; s < S; s++)
+                if (li[s] < ncand)
+                    for (int row = 0; row < J; row++)
+                        a.traj[((long long)k * J + row) * ncand + li[s]] = __int_as_float(0x7fc00000);
+    }
+
+    if (MODE == MODE_BATCH) {
+#pragma unroll
+        for (int s = 0; s < S; s++) {
+            if (li[s] < ncand) {
+                a.steps[li[s]] = steps[s];
+                if (a.safe) a.safe[li[s]] = steps[s] == H ? 1 : 0;
+            }
+        }
+        return;
+    }
+
+    // ---- a5-a7: key, argmin, finalise -------------------------------------------------------------
+    unsigned long long key = kKeyNone;
+    unsigned n_safe = 0, n_exec = 0;
+#pragma unroll
+    for (int s = 0; s < S; s++) {
+        if (li[s] < ncand && inputs_ok) {
+            const bool safe = steps[s] == H;
+            float d2 = 0.f;
+#pragma unroll
+            for (int j = 0; j < M; j++) {
+                const float uj = (s & 1) ? z[s >> 1][D + j].y : z[s >> 1][D + j].x;
+                const float df = __fsub_rn(uj, u_h[j]);
+                d2 = __fmaf_rn(df, df, d2);
+            }
+            const unsigned long long kk = make_key(safe, d2, H, steps[s], cfg.shard_begin + li[s]);
+            key = kk < key ? kk : key;
+            n_safe += safe ? 1u : 0u;
+            n_exec += (unsigned)(steps[s] + 1 < H ? steps[s] + 1 : H);
+        }
+    }
+    block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial);
+}
+
+}  // namespace mpmi

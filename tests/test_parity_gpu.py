@@ -1,0 +1,318 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the FP64 oracle, element by
+element on the same seeded inputs.  Run on the B200 box: python -m pytest tests -m gpu."""
+import copy
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads import generate as G
+from parity_util import traj_rel_err, check_flags, accept_selection, TRAJ_RTOL, MARGIN
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def mp():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1906_02318_b200 as mp
+    mp.load_library()            # raises if the extension is missing: no fallback
+    return mp
+
+
+def _oracle(w, **kw):
+    from oracle.oracle import Oracle
+    return Oracle(w, **kw)
+
+
+def _dev(a, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).cuda()
+
+
+def _small(name, N):
+    w = W.make(name, N=N)
+    if name == "C3":
+        side = int(round(N ** 0.5)); w.N = side * side
+        w.grid_counts = np.array([side, side], np.int32)
+    return w
+
+
+# ------------------------------------------------------------------ a1: sampler, bit-exact --------
+@pytest.mark.parametrize("name", ["C1", "C3", "C5"])
+def test_sampler_bit_exact(mp, name):
+    """K = 0 and B = [I_m; 0] make z_1[0:m] = u exactly, so the lifted dump of step 1 exposes the
+    kernel's own candidates: they must equal the oracle's bit for bit (Philox and grid)."""
+    w = _small(name, 1500 if name != "C3" else 1600)
+    w.K = np.zeros_like(w.K); w.B = np.zeros_like(w.B)
+    for j in range(w.m):
+        w.B[j, j] = 1.0
+    w.u_lo = np.array([-1.0, 0.0, -1.0][: w.m], np.float32); w.u_hi = np.array([1.0, 1.0, 0.0][: w.m], np.float32)
+    w.seed = 0xDEADBEEF12345
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    N = w.N
+    X0 = _dev(w.x_nom[None, :])
+    traj = torch.empty((1, w.d, N), dtype=torch.float32, device="cuda")
+    steps = torch.empty(N, dtype=torch.int32, device="cuda")
+    for tick in (0, (5 << 32) | 77):
+        ctx.rollout_batch(0, X0.data_ptr(), 1, N, 1, mp.DUMP_LIFTED, traj.data_ptr(), steps.data_ptr(), 0, tick=tick)
+        torch.cuda.synchronize()
+        got = traj[0, : w.m, :].T.cpu().numpy()
+        ref = o.sample(tick, np.arange(N))
+        assert np.array_equal(got.view(np.uint32), ref.view(np.uint32))
+
+
+# ------------------------------------------------------------------ a2: lift ------------------------
+@pytest.mark.parametrize("name", ["C2", "C3", "C5"])
+def test_lift_parity(mp, name):
+    """K = I, B = 0, H = 1  =>  z_1 = Psi(x0) exactly; per-candidate x0."""
+    w = _small(name, 300 if name != "C3" else 289)
+    w.K = np.eye(w.d, dtype=np.float32); w.B = np.zeros_like(w.B)
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    x0s, _, _ = W.tick_inputs(w, w.N)
+    x0s = (x0s * 3.0).astype(np.float32)
+    U = np.zeros((w.N, w.m), np.float32)
+    traj = torch.empty((1, w.d, w.N), dtype=torch.float32, device="cuda")
+    steps = torch.empty(w.N, dtype=torch.int32, device="cuda")
+    dU, dX = _dev(U), _dev(x0s)                    # keep the tensors alive while the kernel runs
+    ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), w.N, w.N, 1, mp.DUMP_LIFTED, traj.data_ptr(),
+                      steps.data_ptr(), 0)
+    torch.cuda.synchronize()
+    got = traj[0].T.cpu().numpy().astype(np.float64)
+    for i in range(w.N):
+        ref = o.lift(x0s[i].astype(np.float64))
+        assert np.all(np.abs(got[i] - ref) <= 2e-6 * np.maximum(np.abs(ref), 1.0)), (i, np.abs(got[i] - ref).max())
+
+
+# ------------------------------------------------------------------ a3/a4/a9: rollouts ---------------
+@pytest.mark.parametrize("name,N,per_cand_x0", [("C1", 1100, False), ("C1", 2500, True), ("C2", 1300, False),
+                                                ("C3", 1000, True), ("C4", 777, False), ("C5", 700, False),
+                                                ("C5", 300, True)])
+def test_rollout_batch_parity(mp, name, N, per_cand_x0):
+    """T1 trajectories (rel. error <= 1e-4), T2 flags (identical where margin > 1e-4), NaN tail."""
+    w = W.make(name, N=N)
+    if name == "C3":
+        w.sampler = 0; w.grid_counts = None
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    rng = np.random.default_rng(11)
+    U = rng.uniform(w.u_lo, w.u_hi, (N, w.m)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, N if per_cand_x0 else 1)
+    H = w.H
+    for kind, J in ((mp.DUMP_LIFTED, w.d), (mp.DUMP_PHYS, w.n)):
+        traj = torch.full((H, J, N), 7.0, dtype=torch.float32, device="cuda")
+        steps = torch.empty(N, dtype=torch.int32, device="cuda")
+        safe = torch.empty(N, dtype=torch.uint8, device="cuda")
+        dU, dX = _dev(U), _dev(x0s)
+        ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), x0s.shape[0], N, H, kind, traj.data_ptr(),
+                          steps.data_ptr(), safe.data_ptr())
+        torch.cuda.synchronize()
+        g_steps = steps.cpu().numpy(); g_safe = safe.cpu().numpy(); g_traj = traj.cpu().numpy()
+        r_steps, r_marg, r_traj = o.rollout_batch(U, x0s, want_traj=True)
+        bad, nrobust = check_flags(g_steps, r_steps, r_marg, H)
+        assert len(bad) == 0, (bad[:5], g_steps[bad[:5]], r_steps[bad[:5]], r_marg[bad[:5]])
+        assert nrobust > 0.9 * N
+        assert np.array_equal(g_safe, (g_steps == H).astype(np.uint8))
+        assert 0.05 < (r_steps == H).mean() < 0.95                    # a mixed set: both branches exercised
+        worst = 0.0
+        for i in range(N):
+            gt = g_traj[:, :, i]
+            e_ref = min(r_steps[i] + 1, H); e_gpu = min(g_steps[i] + 1, H)
+            worst = max(worst, traj_rel_err(gt, r_traj[i][:, :J] if kind == mp.DUMP_PHYS else r_traj[i], min(e_ref, e_gpu))
+                        if kind == mp.DUMP_LIFTED else 0.0)
+            if kind == mp.DUMP_PHYS:
+                e = min(e_ref, e_gpu)
+                assert np.allclose(gt[:e], r_traj[i][:e, : w.n], rtol=1e-4, atol=1e-4)
+            assert np.all(np.isfinite(gt[:e_gpu])) and np.all(np.isnan(gt[e_gpu:]))
+        assert worst <= TRAJ_RTOL, worst
+
+
+# ------------------------------------------------------------------ a1-a8: whole tick ----------------
+def _tick_compare(mp, w, nticks, expect=None):
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    x0s, uus, ticks = W.tick_inputs(w, nticks)
+    exact = 0
+    branches = set()
+    for x0, uu, t in zip(x0s, uus, ticks):
+        ref = o.step(x0, uu, int(t), detail=True)
+        r = ctx.step_sync(x0, uu, int(t)).as_dict(w.m)
+        ok, ex, why = accept_selection(r, ref, w.H)
+        assert ok, (why, r, {k: ref[k] for k in ("index", "safe", "steps", "dist")})
+        exact += ex
+        robust = ref["margin_all"] > MARGIN
+        if robust.all():
+            assert r["n_safe"] == ref["n_safe"] and r["n_exec"] == ref["n_exec"]
+        else:
+            assert abs(r["n_safe"] - ref["n_safe"]) <= (~robust).sum()
+        if ex:
+            assert abs(r["dist"] - ref["dist"]) <= 1e-6 * max(1.0, ref["dist"])
+        branches.add("user" if (r["safe"] and r["dist"] == 0) else "intervene" if r["safe"] else "fallback")
+    if expect:
+        assert branches == expect, branches
+    return exact / nticks, branches
+
+
+@pytest.mark.parametrize("name,N", [("C1", 1024), ("C2", 10000), ("C3", 10000), ("C4", 1 << 14), ("C5", 2048)])
+def test_tick_parity(mp, name, N):
+    """T3 over 64 (C5: 16) seeded ticks: minimal-intervention and intervention branches."""
+    w = W.make(name, N=N)
+    rate, branches = _tick_compare(mp, w, 64 if name != "C5" else 16)
+    assert rate >= 0.95, rate
+    assert "intervene" in branches
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5"])
+def test_tick_forced_branches(mp, name):
+    """bounds x0.01 -> nothing is safe (fallback rule G1); bounds x100 -> everything is safe."""
+    w = W.make(name, N=1500 if name != "C3" else 1600)
+    if name == "C3":
+        w.grid_counts = np.array([40, 40], np.int32)
+    _, b = _tick_compare(mp, G.scaled_bounds(w, 0.01), 8)
+    assert b == {"fallback"}
+    _, b = _tick_compare(mp, G.scaled_bounds(w, 100.0), 8)
+    assert b == {"user"}
+
+
+def test_c2_tick_sequence_replay(mp):
+    """C2: 1,000 consecutive ticks with u_user from a random walk (BASELINE.json configs[1]); the GPU
+    replays the stored sequence; every 10th tick is compared with the oracle in full."""
+    w = W.make("C2")
+    seq = np.loadtxt(W.generate.C2_SEQUENCE, comments="#")
+    assert seq.shape == (1000, 9)
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    exact = 0
+    kinds = set()
+    for row in seq:
+        t = int(row[0]); x0 = row[1:5].astype(np.float32); uu = row[5:6].astype(np.float32)
+        r = ctx.step_sync(x0, uu, t).as_dict(1)
+        same = (r["index"], r["safe"], r["steps"]) == (int(row[6]), int(row[7]), int(row[8]))
+        exact += same
+        if not same or t % 10 == 0:              # every mismatch and every 10th tick: full oracle comparison
+            ref = o.step(x0, uu, t, detail=True)
+            assert (ref["index"], ref["safe"], ref["steps"]) == (int(row[6]), int(row[7]), int(row[8]))
+            ok, ex, why = accept_selection(r, ref, w.H)
+            assert ok, (t, why)
+        kinds.add("user" if (r["safe"] and r["dist"] == 0) else "intervene" if r["safe"] else "fallback")
+    assert exact >= 950, exact
+    assert kinds >= {"user", "intervene"}
+
+
+# ------------------------------------------------------------------ entry-point equivalences ---------
+def test_device_and_shard_paths_match_host_path(mp):
+    """mpmi_step_device == mpmi_step_sync; two shards + finalize == one context (P7 shard invariance)."""
+    for name in ("C2", "C5"):
+        w = W.make(name, N=3000)
+        ctx = mp.Context(w)
+        cut = 1234
+        sh = [mp.Context(w, shard=(0, cut)), mp.Context(w, shard=(cut, w.N + 1 - cut))]
+        x0s, uus, ticks = W.tick_inputs(w, 6)
+        d_res = torch.zeros(56, dtype=torch.uint8, device="cuda")
+        d_parts = torch.zeros(2 * 24, dtype=torch.uint8, device="cuda")
+        s = torch.cuda.current_stream().cuda_stream
+        for x0, uu, t in zip(x0s, uus, ticks):
+            host = ctx.step_sync(x0, uu, int(t)).as_dict(w.m)
+            dx, du = _dev(x0), _dev(uu)
+            ctx.step_device(dx.data_ptr(), du.data_ptr(), int(t), s, d_res.data_ptr())
+            torch.cuda.synchronize()
+            dev = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)[0]
+            for g in range(2):
+                sh[g].shard_step(dx.data_ptr(), du.data_ptr(), int(t), s, d_parts.data_ptr() + 24 * g)
+            sh[0].shard_finalize(d_parts.data_ptr(), 2, du.data_ptr(), int(t), s, d_res.data_ptr())
+            torch.cuda.synchronize()
+            shd = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)[0]
+            for got in (dev, shd):
+                assert got["index"] == host["index"] and got["safe"] == host["safe"] and got["steps"] == host["steps"]
+                assert got["n_safe"] == host["n_safe"] and got["n_exec"] == host["n_exec"] and got["key"] == host["key"]
+                assert np.array_equal(got["u"][: w.m], host["u"]) and got["dist"] == host["dist"]
+
+
+def test_edge_cases(mp):
+    w = W.make("C1", N=1)
+    o = _oracle(w)
+    for inc in (0, 1):
+        ctx = mp.Context(w, include_user=inc)
+        oo = _oracle(w, include_user=inc)
+        r = ctx.step_sync(w.x_nom, np.array([0.2], np.float32), 3).as_dict(1)
+        ref = oo.step(w.x_nom, np.array([0.2], np.float32), 3, detail=True)
+        assert accept_selection(r, ref, w.H)[0]
+    # u_user outside the box is clamped, not an error
+    w = W.make("C2", N=512)
+    ctx = mp.Context(w); o = _oracle(w)
+    r = ctx.step_sync(w.x_nom, np.array([7.5], np.float32), 1).as_dict(1)
+    ref = o.step(w.x_nom, np.array([7.5], np.float32), 1, detail=True)
+    assert accept_selection(r, ref, w.H)[0] and ref["U"][w.N, 0] == 1.0
+    # non-finite inputs: INVALID on the host path, index -1 on the device path
+    with pytest.raises(mp.MpmiError) as e:
+        ctx.step_sync(np.array([np.nan, 0, 0, 0], np.float32), np.array([0.0], np.float32), 0)
+    assert e.value.status == -1
+    d_res = torch.zeros(56, dtype=torch.uint8, device="cuda")
+    dx, du = _dev(np.array([np.inf, 0, 0, 0], np.float32)), _dev(np.zeros(1, np.float32))
+    ctx.step_device(dx.data_ptr(), du.data_ptr(), 0, 0, d_res.data_ptr())
+    torch.cuda.synchronize()
+    assert np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)[0]["index"] == -1
+    r2 = ctx.step_sync(w.x_nom, np.array([7.5], np.float32), 1).as_dict(1)       # state was reset correctly
+    assert r2["index"] == r["index"] and r2["n_exec"] == r["n_exec"]
+    # H = 1, candidates an exact multiple of the CTA tile, inflated barrier
+    w = W.make("C5", N=511, H=1); w.inflate = 0.05
+    ctx = mp.Context(w); o = _oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        assert accept_selection(ctx.step_sync(x0, uu, int(t)).as_dict(3), o.step(x0, uu, int(t), detail=True), 1)[0]
+    # unsupported sizes are statuses
+    bad = dict(vars(W.make("C1"))); bad["m"] = 5
+    with pytest.raises(mp.MpmiError) as e:
+        mp.Context(bad)
+    assert e.value.status == -2
+
+
+# ------------------------------------------------------------------ full size, bench launch config ---
+@pytest.mark.parametrize("name", ["C4", "C5"])
+def test_full_size_sampled(mp, name):
+    """BASELINE sizes (C4: N = 2^20, C5: N = 262,144) in the launch configuration bench.py times:
+    the tick result against oracle rollouts of sampled candidates, plus size-independent properties."""
+    w = W.make(name)
+    o = _oracle(w, N=w.N)
+    ctx = mp.Context(w)
+    N, H = w.N, w.H
+    x0s, uus, ticks = W.tick_inputs(w, 2)
+    steps = torch.empty(N, dtype=torch.int32, device="cuda")
+    rng = np.random.default_rng(3)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        r = ctx.step_sync(x0, uu, int(t)).as_dict(w.m)
+        dX = _dev(x0[None, :])
+        ctx.rollout_batch(0, dX.data_ptr(), 1, N, H, mp.DUMP_NONE, 0, steps.data_ptr(), 0, tick=int(t))
+        torch.cuda.synchronize()
+        g_steps = steps.cpu().numpy()
+        u_h = np.clip(uu, w.u_lo, w.u_hi)
+        z0 = o.lift(x0.astype(np.float64))
+        us, _, _ = o.rollout(z0, u_h.astype(np.float64))
+        n_safe = int((g_steps == H).sum()) + int(us == H)
+        n_exec = int(np.minimum(g_steps + 1, H).sum()) + min(us + 1, H)
+        assert abs(r["n_safe"] - n_safe) <= 1 and abs(r["n_exec"] - n_exec) <= H      # tick == batch + user slot
+        assert 0.2 < n_safe / N < 0.6
+        idx = np.unique(np.concatenate([rng.integers(0, N, 1500), [r["index"]] if r["index"] < N else []])).astype(np.int64)
+        Us = o.sample(int(t), idx)
+        r_steps, r_marg, _ = o.rollout_batch(Us, x0[None, :])
+        robust = r_marg > MARGIN
+        assert np.array_equal(g_steps[idx][robust], r_steps[robust]) and robust.mean() > 0.9
+        # winner: bit-identical to its candidate, safe in the oracle, and no sampled robustly safe candidate is closer
+        if r["index"] < N:
+            assert np.array_equal(r["u"], o.sample(int(t), [r["index"]])[0])
+        else:
+            assert np.array_equal(r["u"], u_h)
+        assert r["safe"] == 1
+        d = np.linalg.norm(Us.astype(np.float64) - u_h.astype(np.float64), axis=1)
+        rs = robust & (r_steps == H)
+        assert not (d[rs] < r["dist"] - MARGIN).any()
+        # brute-force check of the argmin on the GPU's own flags (exact, all N candidates)
+        Uall_d = None
+        if name == "C4":
+            Uall = o.sample(int(t), np.arange(0, N, 1)[:: 1][: 1 << 15])
+            dd = np.linalg.norm(Uall.astype(np.float64) - u_h.astype(np.float64), axis=1)
+            ok = g_steps[: 1 << 15] == H
+            if ok.any() and us != H:
+                assert dd[ok].min() >= r["dist"] - 1e-6

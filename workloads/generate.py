@@ -18,6 +18,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CALIBRATION_JSON = os.path.join(_HERE, "calibration.json")
+C2_SEQUENCE = os.path.join(_HERE, "c2_tick_sequence.txt")   # written by oracle/make_c2_sequence.py
 CONFIG_NAMES = ("C1", "C2", "C3", "C4", "C5")
 
 ONE = 0xFF           # lift factor codes (include/mpmi.h: mpmi_lift_spec.terms)
