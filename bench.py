@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200-native MPMI-SC tick (BASELINE.json metric:
+"rollout sample-steps/sec and p50/p99 per-tick latency at N=10k and 1M; % FP32 peak").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4] [--impl reference]
+
+One "step" is one whole control tick: sample N candidates -> lift ->
+H-step rollout with per-step safe test -> argmin selection -> result, on one batch of synthetic
+input (a fresh x0, u_user and Philox tick per step).  Default workload: C4 at N = 2^20, H = 100
+(BASELINE.json configs[3], the configuration the throughput half of the metric is quoted on);
+the latency half (p50/p99 at N = 10k, C2, and at N = 2^20) is reported under "latency".
+
+value    = executed sample-steps/s with inputs resident in HBM (mpmi_step_device), CUDA-event timed
+e2e      = the same metric through mpmi_step_sync with HOST buffers (H2D + D2H inside the region)
+roofline = the rollout kernel against the FP32 FMA peak ("alu")
+cpu_baseline = the FP64 oracle, as it stands, on this box's host cores (bounded sample)
+
+One "sample-step" = one evaluation of z <- K z + B u followed by isSafe; candidate i executes
+min(steps_i + 1, H) of them (Algorithm 2 l.4 stops at the first violation).  The nominal N*H count
+is reported beside it.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.45: SMs x FP32 lanes x 2 flop x max SM clock
+
+
+def _flop_per_sample_step(w):
+    return 2.0 * w.d * (w.d + w.m)                      # dense K and B, nothing discounted
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi style clock / throttle-reason samples DURING the timed region (NVML)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag = index, [], False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                mx = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+                rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                self.samples.append((sm, mx, rs))
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap", nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        seen = set()
+        for _, _, rs in self.samples:
+            for bit, name in names.items():
+                if rs & bit:
+                    seen.add(name)
+        sm = sorted(s[0] for s in self.samples)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": self.samples[0][1], "reasons": sorted(seen),
+                "samples": len(sm)}
+
+
+def _percentiles(v):
+    v = np.sort(np.asarray(v, dtype=np.float64))
+    return float(v[len(v) // 2]), float(v[min(len(v) - 1, int(0.99 * len(v)))])
+
+
+def run_reference(args):
+    """--impl reference: the FP64 oracle as it stands, on the host cores, same config / metric / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import workloads as W
+    from oracle import oracle as O
+    w = W.make(args.workload, N=args.N)
+    x0s, uus, ticks = W.tick_inputs(w, args.warmup + args.steps)
+    # bounded sample: the first n_ref candidates of the same workload, sized from one probe tick
+    n_ref = min(w.N, 1 << 14)
+    t0 = time.perf_counter()
+    r = O.Oracle(w, N=n_ref).step(x0s[0], uus[0], 0)
+    rate = r["n_exec"] / (time.perf_counter() - t0)
+    budget_s = 150.0 / max(1, args.steps + args.warmup)
+    n_ref = int(min(w.N, max(1 << 12, rate * budget_s / (w.H * 0.7))))
+    o = O.Oracle(w, N=n_ref)
+    for t in range(args.warmup):
+        o.step(x0s[t], uus[t], int(ticks[t]))
+    n_exec, t0 = 0, time.perf_counter()
+    for t in range(args.warmup, args.warmup + args.steps):
+        n_exec += o.step(x0s[t], uus[t], int(ticks[t]))["n_exec"]
+    dt = time.perf_counter() - t0
+    val = n_exec / dt
+    sample = f"first {n_ref} of {w.N} candidates (+ user slot) per tick, {args.steps} ticks, H={w.H}"
+    print(json.dumps({
+        "impl": "reference", "metric": "rollout sample-steps/s", "value": val, "unit": "sample-steps/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: n={w.n} m={w.m} d={w.d} N={w.N} H={w.H}", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "sample-steps/s", "cores": O.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "sample-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--N", type=int, default=None, help="override candidates per GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-latency", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import workloads as W
+    import paper_1906_02318_b200 as mp
+    mp.load_library()                                        # fails loudly if the CUDA extension is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # ---- workload: weak scaling -- every rank owns N_per candidates of a global set of world*N_per
+    w1 = W.make(args.workload, N=args.N)
+    n_per = w1.N
+    w = W.make(args.workload, N=n_per * world)
+    K_, W_ = args.steps, args.warmup
+    x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
+    from paper_1906_02318_b200.shard import shard_plan, gather_partials
+    begin, count = shard_plan(w.N, 1, world, rank)             # the injected u_user (index N) goes to the last rank
+    ctx = mp.Context(w, device=local, shard=(begin, count) if world > 1 else (0, 0))
+    info = ctx.info()
+    stream = torch.cuda.current_stream().cuda_stream
+
+    dX0 = torch.as_tensor(x0s).cuda().contiguous()
+    dUU = torch.as_tensor(uus).cuda().contiguous()
+    dRes = torch.zeros((W_ + K_, 56), dtype=torch.uint8, device="cuda")
+    dPart = torch.zeros(3, dtype=torch.int64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    def tick_device(t):
+        px, pu, pr = dX0[t].data_ptr(), dUU[t].data_ptr(), dRes[t].data_ptr()
+        if world == 1:
+            ctx.step_device(px, pu, int(ticks[t]), stream, pr)
+        else:                                                  # shard -> 24-byte all-gather -> finalise
+            ctx.shard_step(px, pu, int(ticks[t]), stream, dPart.data_ptr())
+            parts = gather_partials(dPart, world)
+            ctx.shard_finalize(parts.data_ptr(), world, pu, int(ticks[t]), stream, pr)
+
+    for t in range(W_):
+        tick_device(t)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K_)]
+    torch.cuda.synchronize()
+    for i in range(K_):
+        flush.fill_(i & 0xFF)                                  # L2 flush between timed iterations (untimed)
+        ev[i][0].record()
+        tick_device(W_ + i)
+        ev[i][1].record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    clocks.stop_flag = True
+    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    total_ms = float(step_ms.sum())
+    res = np.frombuffer(dRes.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)
+    n_exec = int(res["n_exec"][W_:].sum())                     # whole-job executed sample-steps (all shards)
+    if dist:
+        tmax = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        total_ms = float(tmax.item())
+    nominal = float(w.N + 1) * w.H * K_
+    value = n_exec / (total_ms * 1e-3)
+
+    # ---- e2e: the public host API, host buffers, H2D + D2H inside the timed region (N = 1 only)
+    e2e = None
+    lat = {}
+    if world == 1:
+        r = mp.Result()
+        x0c = [np.ascontiguousarray(x) for x in x0s]; uuc = [np.ascontiguousarray(u) for u in uus]
+        for t in range(W_):
+            ctx.step_sync(x0c[t], uuc[t], int(ticks[t]), stream)
+        torch.cuda.synchronize()
+        e_exec, wall = 0, []
+        t_all = time.perf_counter()
+        for t in range(W_, W_ + K_):
+            t0 = time.perf_counter()
+            rr = ctx.step_sync(x0c[t], uuc[t], int(ticks[t]), stream)
+            wall.append(time.perf_counter() - t0)
+            e_exec += rr.n_exec
+        t_all = time.perf_counter() - t_all
+        e2e = {"value": e_exec / t_all, "unit": "sample-steps/s", "h2d_bytes_per_step": 112, "d2h_bytes_per_step": 56,
+               "ms_per_step": 1e3 * t_all / K_}
+        p50, p99 = _percentiles(wall)
+        lat[f"{args.workload}_N{w.N}"] = {"host_p50_us": 1e6 * p50, "host_p99_us": 1e6 * p99,
+                                          "gpu_p50_us": 1e3 * _percentiles(step_ms)[0], "ticks": K_}
+        if not args.no_latency:
+            # latency half of the metric: C2 (N = 10k), 1,000 stored closed-loop ticks, host API
+            w2 = W.make("C2")
+            seq = np.loadtxt(W.generate.C2_SEQUENCE, comments="#")
+            c2 = mp.Context(w2, device=local)
+            xs = [np.ascontiguousarray(row[1:5], dtype=np.float32) for row in seq]
+            us = [np.ascontiguousarray(row[5:6], dtype=np.float32) for row in seq]
+            for t in range(50):
+                c2.step_sync(xs[t], us[t], t, stream)
+            wall = []
+            for t in range(len(seq)):
+                t0 = time.perf_counter()
+                c2.step_sync(xs[t], us[t], t, stream)
+                wall.append(time.perf_counter() - t0)
+            p50, p99 = _percentiles(wall)
+            lat["C2_N10000"] = {"host_p50_us": 1e6 * p50, "host_p99_us": 1e6 * p99, "ticks": len(seq)}
+            c2.close()
+
+    # ---- roofline of the dominant (only) kernel: plain FP32 FMA arithmetic
+    flop = _flop_per_sample_step(w)
+    achieved = n_exec / world * flop / (total_ms * 1e-3) / 1e12            # per GPU
+    traffic = None
+    tj = os.path.join(ROOT, "profiles", "roofline_traffic.csv")     # ncu --set full, dram bytes per launch
+    if os.path.exists(tj):
+        for line in open(tj).read().splitlines()[1:]:
+            f = line.split(",")
+            if f and f[0] == args.workload:
+                traffic = int(f[2])
+    roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
+                "kernel": "rollout_reg_kernel" if info["variant"] == 1 else "rollout_tile_kernel",
+                "nominal_frac": nominal / K_ / max(world, 1) * flop / (total_ms * 1e-3 / K_) / 1e12 / FP32_PEAK_TFLOPS}
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    # ---- CPU baseline: the oracle as it stands on this box's host cores (bounded sample)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as O
+        n_s = min(w.N, 1 << 18)
+        o = O.Oracle(w, N=n_s)
+        o.step(x0s[0], uus[0], 0)
+        ne, t0, nt = 0, time.perf_counter(), 0
+        while time.perf_counter() - t0 < 10.0 and nt < K_:
+            ne += o.step(x0s[W_ + nt], uus[W_ + nt], int(ticks[W_ + nt]))["n_exec"]; nt += 1
+        dt = time.perf_counter() - t0
+        cpu = {"value": ne / dt, "unit": "sample-steps/s", "cores": O.num_threads(), "kind": "oracle",
+               "sample": f"first {n_s} of {w.N} candidates (+ user slot), {nt} ticks, H={w.H}, fp64"}
+
+    out = {
+        "metric": "rollout sample-steps/s", "value": value, "unit": "sample-steps/s", "n_gpus": world,
+        "steps": K_, "warmup": W_, "ms_per_step": total_ms / K_, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: n={w.n} m={w.m} d={w.d} N={n_per}/GPU (+1 user slot) H={w.H}, "
+                               f"Philox/grid sampler, calibrated 40% safe (DESIGN.md section 4)",
+                   "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
+                   "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if world > 1 else "single GPU",
+                   "kernel": info},
+        "nominal_value": nominal / (total_ms * 1e-3), "executed_fraction": n_exec / nominal,
+        "safe_fraction": float(res["n_safe"][W_:].mean() / (w.N + 1)),
+        "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": K_ * (1 if world == 1 else 2),
+        "roofline": roofline, "cpu_baseline": cpu, "latency": lat,
+        "paper_context": "paper: >10,000 trajectories per tick at ~100 Hz / ~60 Hz on a GeForce 860M (PAPER.md:12, 266)",
+    }
+    print(json.dumps(out))
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
