@@ -51,6 +51,11 @@ typedef enum {
 enum { MPMI_SAMPLER_PHILOX = 0, MPMI_SAMPLER_GRID = 1 };
 enum { MPMI_LIFT_MONO = 0, MPMI_LIFT_RFF = 1 };
 enum { MPMI_DUMP_NONE = 0, MPMI_DUMP_PHYS = 1, MPMI_DUMP_LIFTED = 2 };
+/* mpmi_config.variant: results never depend on these, only speed does */
+enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)                  */
+       MPMI_VARIANT_WIDE = 2,           /* 64/D candidates per thread (throughput)            */
+       MPMI_VARIANT_NO_BINNING = 4,     /* never order the Philox candidates spatially        */
+       MPMI_VARIANT_FORCE_BINNING = 8 };/* order them even for small N                        */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:
@@ -96,7 +101,7 @@ typedef struct {
     /* Candidate sharding across GPUs: this context owns the global candidate
      * indices [shard_begin, shard_begin + shard_count) of the N (+1) candidates; 0,0 = all of them. */
     int64_t  shard_begin, shard_count;
-    int32_t  variant;         /* 0 = automatic kernel choice; see mpmi_info.variant                */
+    int32_t  variant;         /* 0 = automatic; else OR of MPMI_VARIANT_* (benchmark / test knobs)  */
     int32_t  reserved;
 } mpmi_config;
 
@@ -125,6 +130,8 @@ typedef struct {
     int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = CTA-tile FFMA2 (d<=128)   */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;
+    int32_t  binning_cells;   /* 0 = candidates walked in index order; else cells of the spatial pre-sort */
+    int32_t  reserved;
     int64_t  ncand_local;     /* candidates this context rolls out per tick                         */
 } mpmi_info;
 

@@ -15,6 +15,8 @@ struct KArgs {
     TickState *st;
     mpmi_result *out;
     mpmi_partial *partial;
+    const int *perm;                      // device, spatial order of the local sampled candidates, or null
+    long long nsamp;                      // sampled candidates of this shard (perm entries)
     // batch
     const float *U;                       // device Ncand*m or null
     long long x0_count;

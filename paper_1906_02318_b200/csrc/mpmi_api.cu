@@ -13,6 +13,7 @@
 #include "../../include/mpmi.h"
 #include "mpmi_device.cuh"
 #include "kernel_args.cuh"
+#include "binning.cuh"
 
 using namespace mpmi;
 
@@ -31,6 +32,11 @@ struct mpmi_ctx {
     cudaGraphExec_t exec = nullptr;
     cudaEvent_t done = nullptr;
     bool pending = false;
+    // spatial binning of Philox candidates (binning.cuh)
+    bool binning = false;
+    BinArgs bin{};
+    int *d_hist = nullptr, *d_cursor = nullptr, *d_perm = nullptr;
+    unsigned *d_bin_ticket = nullptr;
     std::string err;
 };
 
@@ -104,6 +110,21 @@ void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a, cudaS
     cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)c->block), args, (size_t)c->smem, s);
 }
 
+// one tick on stream s: [cell histogram + scan, scatter] (large Philox sets only) -> fused tick kernel
+void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
+    if (c->binning) {
+        BinArgs b = c->bin;
+        b.tick_ptr = a.tick_ptr; b.tick_val = a.tick_val;
+        long long g = (b.nsamp + 255) / 256;
+        const long long gmax = 8LL * c->sm_count;
+        const unsigned grid = (unsigned)(g < gmax ? g : gmax);
+        bin_hist_kernel<<<grid, 256, 0, s>>>(c->dc, b);
+        bin_scatter_kernel<<<grid, 256, 0, s>>>(c->dc, b);
+        a.perm = c->d_perm; a.nsamp = b.nsamp;
+    }
+    launch(c, c->k_tick, c->dc.shard_count, a, s);
+}
+
 int build_graph(mpmi_ctx *c) {
     cudaStream_t s;
     CU(c, cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
@@ -112,7 +133,7 @@ int build_graph(mpmi_ctx *c) {
     a.st = c->d_state; a.out = c->d_res;
     CU(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     cudaMemcpyAsync(c->d_in, c->h_in, sizeof(TickIn), cudaMemcpyHostToDevice, s);
-    launch(c, c->k_tick, c->dc.shard_count, a, s);
+    enqueue_tick(c, a, s);
     cudaMemcpyAsync(c->h_res, c->d_res, sizeof(mpmi_result), cudaMemcpyDeviceToHost, s);
     CU(c, cudaStreamEndCapture(s, &c->graph));
     CU(c, cudaGraphInstantiate(&c->exec, c->graph, 0));
@@ -145,6 +166,7 @@ void mpmi_destroy(mpmi_ctx *c) {
     if (c->graph) cudaGraphDestroy(c->graph);
     cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
     cudaFree(c->d_in); cudaFree(c->d_state); cudaFree(c->d_res);
+    cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_in); cudaFreeHost(c->h_res);
     delete c;
 }
@@ -298,13 +320,36 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     std::memset(c->h_in, 0, sizeof(TickIn));
     CUC(cudaEventCreateWithFlags(&c->done, cudaEventDisableTiming));
 
+    // ---- spatial binning: large Philox candidate sets only (the grid is already spatially ordered)
+    {
+        const long long send = sb + sc < cfg->N ? sb + sc : cfg->N;
+        const long long nsamp = send > sb ? send - sb : 0;
+        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (1 << 15);
+        c->binning = (cfg->variant & MPMI_VARIANT_FORCE_BINNING) ? (cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= 64)
+                                                                  : (want && !(cfg->variant & MPMI_VARIANT_NO_BINNING));
+        if (c->binning) {
+            int total = 0;
+            while ((64LL << (total + 1)) <= nsamp && total < 16) total++;      // ~64 candidates per cell
+            for (int t = 0; t < total; t++) c->bin.bits[t % m]++;
+            c->bin.ncells = 1 << total;
+            c->bin.nsamp = nsamp;
+            CUC(cudaMalloc(&c->d_hist, sizeof(int) * c->bin.ncells));
+            CUC(cudaMemset(c->d_hist, 0, sizeof(int) * c->bin.ncells));
+            CUC(cudaMalloc(&c->d_cursor, sizeof(int) * c->bin.ncells));
+            CUC(cudaMalloc(&c->d_perm, sizeof(int) * nsamp));
+            CUC(cudaMalloc(&c->d_bin_ticket, sizeof(unsigned)));
+            CUC(cudaMemset(c->d_bin_ticket, 0, sizeof(unsigned)));
+            c->bin.hist = c->d_hist; c->bin.cursor = c->d_cursor; c->bin.perm = c->d_perm; c->bin.ticket = c->d_bin_ticket;
+        }
+    }
+
     // ---- kernel choice ------------------------------------------------------------------------------
     if (D <= 32) {
         c->variant = 1;
         const int Pmax = 32 / D;
         // enough warps to give every SM sub-partition two warps at the wide packing?  else 2 cand/thread
         const long long warps_wide = (sc + 2LL * Pmax * 32 - 1) / (2LL * Pmax * 32);
-        c->P = (cfg->variant == 11) ? 1 : (cfg->variant == 12) ? Pmax : (warps_wide >= 8LL * c->sm_count ? Pmax : 1);
+        c->P = (cfg->variant & MPMI_VARIANT_NARROW) ? 1 : (cfg->variant & MPMI_VARIANT_WIDE) ? Pmax : (warps_wide >= 8LL * c->sm_count ? Pmax : 1);
         const long long threads = (sc + 2LL * c->P - 1) / (2LL * c->P);
         c->block = threads >= 128LL * 2 * c->sm_count ? 128 : threads >= 64LL * 2 * c->sm_count ? 64 : 32;
         c->cand_per_block = 2 * c->P * c->block;
@@ -339,7 +384,8 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->threads_per_block = c->block;
     o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
-    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = 1; o->uses_graph = 1;
+    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = c->binning ? 3 : 1; o->uses_graph = 1;
+    o->binning_cells = c->binning ? c->bin.ncells : 0;
     o->ncand_local = c->dc.shard_count;
     return MPMI_OK;
 }
@@ -382,7 +428,7 @@ int mpmi_step_device(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint
     KArgs a{};
     a.x0 = d_x0; a.u_user = d_u_user; a.tick_ptr = nullptr; a.tick_val = tick;
     a.st = c->d_state; a.out = d_out;
-    launch(c, c->k_tick, c->dc.shard_count, a, (cudaStream_t)stream);
+    enqueue_tick(c, a, (cudaStream_t)stream);
     CU(c, cudaGetLastError());
     return MPMI_OK;
 }
@@ -394,7 +440,7 @@ int mpmi_shard_step(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint6
     KArgs a{};
     a.x0 = d_x0; a.u_user = d_u_user; a.tick_ptr = nullptr; a.tick_val = tick;
     a.st = c->d_state; a.out = nullptr; a.partial = d_partial;
-    launch(c, c->k_tick, c->dc.shard_count, a, (cudaStream_t)stream);
+    enqueue_tick(c, a, (cudaStream_t)stream);
     CU(c, cudaGetLastError());
     return MPMI_OK;
 }

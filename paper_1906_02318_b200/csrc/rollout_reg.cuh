@@ -83,6 +83,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
     for (int s = 0; s < S; s++) {
         li[s] = (long long)blockIdx.x * (S * bdim) + s * bdim + tid;
+        if (MODE == MODE_TICK && a.perm && li[s] < a.nsamp) li[s] = a.perm[li[s]];   // spatially ordered walk
         const bool valid = li[s] < ncand && inputs_ok;
         alive[s] = valid;
         steps[s] = 0;

@@ -54,7 +54,8 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
     __syncthreads();
 
     // ---- a1 + a2: thread i fills column i of the tile ----------------------------------------------
-    const long long li = (long long)blockIdx.x * NC + tid;      // kTileThreads == NC
+    long long li = (long long)blockIdx.x * NC + tid;            // kTileThreads == NC
+    if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];   // spatially ordered walk
     bool alive = li < ncand && inputs_ok;
     int steps = 0;
     {

@@ -14,6 +14,7 @@ SAMPLER_PHILOX, SAMPLER_GRID = 0, 1
 LIFT_MONO, LIFT_RFF = 0, 1
 DUMP_NONE, DUMP_PHYS, DUMP_LIFTED = 0, 1, 2
 OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4
+VARIANT_NARROW, VARIANT_WIDE, VARIANT_NO_BINNING, VARIANT_FORCE_BINNING = 1, 2, 4, 8
 
 EXPORTS = ("mpmi_create", "mpmi_destroy", "mpmi_step", "mpmi_step_result", "mpmi_step_sync",
            "mpmi_step_device", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
@@ -69,7 +70,8 @@ class Info(C.Structure):
     _fields_ = [("d_pad", C.c_int32), ("variant", C.c_int32), ("cand_per_block", C.c_int32),
                 ("threads_per_block", C.c_int32), ("blocks", C.c_int32), ("smem_bytes", C.c_int32),
                 ("regs_per_thread", C.c_int32), ("sm_count", C.c_int32), ("launches_per_tick", C.c_int32),
-                ("uses_graph", C.c_int32), ("ncand_local", C.c_int64)]
+                ("uses_graph", C.c_int32), ("binning_cells", C.c_int32), ("reserved", C.c_int32),
+                ("ncand_local", C.c_int64)]
 
 
 _lib = None

@@ -230,6 +230,26 @@ def test_device_and_shard_paths_match_host_path(mp):
                 assert np.array_equal(got["u"][: w.m], host["u"]) and got["dist"] == host["dist"]
 
 
+@pytest.mark.parametrize("name,N", [("C1", 5000), ("C4", 70000), ("C5", 40000)])
+def test_spatial_binning_changes_nothing(mp, name, N):
+    """The counting sort of candidate indices by input-box cell (binning.cuh) only re-orders the walk:
+    every field of the result is identical with and without it, and it matches the oracle."""
+    w = W.make(name, N=N)
+    plain = mp.Context(w, variant=mp.mpmi.VARIANT_NO_BINNING)
+    binned = mp.Context(w, variant=mp.mpmi.VARIANT_FORCE_BINNING)
+    assert plain.info()["binning_cells"] == 0 and binned.info()["binning_cells"] > 1
+    o = _oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 5)
+    for i, (x0, uu, t) in enumerate(zip(x0s, uus, ticks)):
+        a = plain.step_sync(x0, uu, int(t)).as_dict(w.m)
+        b = binned.step_sync(x0, uu, int(t)).as_dict(w.m)
+        for k in ("index", "safe", "steps", "n_safe", "n_exec", "key", "dist"):
+            assert a[k] == b[k], (k, a[k], b[k])
+        assert np.array_equal(a["u"], b["u"])
+        if i < 2:
+            assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
+
+
 def test_edge_cases(mp):
     w = W.make("C1", N=1)
     o = _oracle(w)
