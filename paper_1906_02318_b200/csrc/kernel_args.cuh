@@ -17,6 +17,7 @@ struct KArgs {
     mpmi_partial *partial;
     const int *perm;                      // device, spatial order of the local sampled candidates, or null
     long long nsamp;                      // sampled candidates of this shard (perm entries)
+    unsigned *work;                       // device batch counter of the persistent tile kernel (zero between launches)
     // batch
     const float *U;                       // device Ncand*m or null
     long long x0_count;

@@ -103,9 +103,14 @@ bool all_finite(const float *p, size_t n) {
     return true;
 }
 
-void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a, cudaStream_t s) {
+void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
     long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
     if (blocks < 1) blocks = 1;
+    KArgs a = a0;
+    if (c->variant == 2) {                       // persistent warp-tile kernel: one CTA per SM
+        if (blocks > c->sm_count) blocks = c->sm_count;
+        a.st = c->d_state; a.work = &c->d_state->work;
+    }
     void *args[2] = {(void *)&c->dc, (void *)&a};
     cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)c->block), args, (size_t)c->smem, s);
 }
@@ -312,7 +317,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     CUC(cudaMalloc(&c->d_in, sizeof(TickIn)));
     CUC(cudaMemset(c->d_in, 0, sizeof(TickIn)));
     CUC(cudaMalloc(&c->d_state, sizeof(TickState)));
-    TickState st0{kKeyNone, 0ull, 0u, 0u};
+    TickState st0{kKeyNone, 0ull, 0u, 0u, 0u, 0u};
     CUC(cudaMemcpy(c->d_state, &st0, sizeof st0, cudaMemcpyHostToDevice));
     CUC(cudaMalloc(&c->d_res, sizeof(mpmi_result)));
     CUC(cudaHostAlloc(&c->h_in, sizeof(TickIn), cudaHostAllocDefault));
@@ -383,6 +388,7 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->d_pad = c->dc.D; o->variant = c->variant; o->cand_per_block = c->cand_per_block;
     o->threads_per_block = c->block;
     o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
+    if (c->variant == 2 && o->blocks > c->sm_count) o->blocks = c->sm_count;
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
     o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = c->binning ? 3 : 1; o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;

@@ -50,6 +50,8 @@ struct TickState {
     unsigned long long n_exec;
     unsigned int n_safe;
     unsigned int ticket;
+    unsigned int work;          // next candidate batch of the persistent tile kernel
+    unsigned int pad;
 };
 
 constexpr unsigned long long kKeyNone = 0x7FFFFFFFFFFFFFFFull;
@@ -170,6 +172,11 @@ __device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long v)
     }
     return v;
 }
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += shfl_xor_u64(v, o);
+    return v;
+}
 __device__ __forceinline__ unsigned warp_sum_u32(unsigned v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -209,16 +216,18 @@ __device__ __forceinline__ void decode_result(const DevCfg &cfg, unsigned long l
 
 template <int kWarps>
 __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, unsigned long long key,
-                                                          unsigned n_safe, unsigned n_exec,
+                                                          unsigned n_safe, unsigned long long n_exec,
                                                           unsigned long long tick, const float (&u_h)[kMaxM],
-                                                          TickState *st, mpmi_result *out, mpmi_partial *partial) {
+                                                          TickState *st, mpmi_result *out, mpmi_partial *partial,
+                                                          unsigned *work = nullptr) {
     __shared__ unsigned long long s_key[kWarps];
-    __shared__ unsigned s_safe[kWarps], s_exec[kWarps];
+    __shared__ unsigned s_safe[kWarps];
+    __shared__ unsigned long long s_exec[kWarps];
     __shared__ bool s_last;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     key = warp_min_u64(key);
     n_safe = warp_sum_u32(n_safe);
-    n_exec = warp_sum_u32(n_exec);
+    n_exec = warp_sum_u64(n_exec);
     if (lane == 0) { s_key[warp] = key; s_safe[warp] = n_safe; s_exec[warp] = n_exec; }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -246,6 +255,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                 decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out);
             }
             st->best_key = kKeyNone; st->n_exec = 0ull; st->n_safe = 0u; st->ticket = 0u;   // ready for next tick
+            if (work) *work = 0u;
             __threadfence();
         }
     }
@@ -256,6 +266,26 @@ __device__ __forceinline__ bool finite_inputs(const DevCfg &cfg, const float *x0
     for (int j = 0; j < cfg.n; j++) ok = ok && isfinite(x0[j]);
     for (int j = 0; j < cfg.m; j++) ok = ok && isfinite(u_user[j]);
     return ok;
+}
+
+// acc += k * z on a candidate pair: one FFMA2 (fma.rn.f32x2) with the model value broadcast to both
+// halves.  Written as in-place PTX ("+l") so that ptxas keeps the accumulator where it is; the
+// intrinsic form made it rotate accumulators through MOVs in partially unrolled loops.
+__device__ __forceinline__ void fma2_bcast(float2 &acc, float k, const float2 &z) {
+    unsigned long long kk, zz, aa;
+    asm("mov.b64 %0, {%1,%1};" : "=l"(kk) : "f"(k));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(zz) : "f"(z.x), "f"(z.y));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(aa) : "f"(acc.x), "f"(acc.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(aa) : "l"(kk), "l"(zz));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
+}
+// acc = k * z (first column of a step)
+__device__ __forceinline__ void mul2_bcast(float2 &acc, float k, const float2 &z) {
+    unsigned long long kk, zz, aa;
+    asm("mov.b64 %0, {%1,%1};" : "=l"(kk) : "f"(k));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(zz) : "f"(z.x), "f"(z.y));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(aa) : "l"(kk), "l"(zz));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
 }
 
 __device__ __forceinline__ float4 lds128(unsigned addr) {

@@ -142,16 +142,11 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
                 for (int p = 0; p < P; p++) {
                     const float2 zc = z[p][c];
                     if (c == 0) {
-                        const float2 zero = make_float2(0.f, 0.f);
-                        acc[p][r + 0] = __ffma2_rn(make_float2(kv.x, kv.x), zc, zero);
-                        acc[p][r + 1] = __ffma2_rn(make_float2(kv.y, kv.y), zc, zero);
-                        acc[p][r + 2] = __ffma2_rn(make_float2(kv.z, kv.z), zc, zero);
-                        acc[p][r + 3] = __ffma2_rn(make_float2(kv.w, kv.w), zc, zero);
+                        mul2_bcast(acc[p][r + 0], kv.x, zc); mul2_bcast(acc[p][r + 1], kv.y, zc);
+                        mul2_bcast(acc[p][r + 2], kv.z, zc); mul2_bcast(acc[p][r + 3], kv.w, zc);
                     } else {
-                        acc[p][r + 0] = __ffma2_rn(make_float2(kv.x, kv.x), zc, acc[p][r + 0]);
-                        acc[p][r + 1] = __ffma2_rn(make_float2(kv.y, kv.y), zc, acc[p][r + 1]);
-                        acc[p][r + 2] = __ffma2_rn(make_float2(kv.z, kv.z), zc, acc[p][r + 2]);
-                        acc[p][r + 3] = __ffma2_rn(make_float2(kv.w, kv.w), zc, acc[p][r + 3]);
+                        fma2_bcast(acc[p][r + 0], kv.x, zc); fma2_bcast(acc[p][r + 1], kv.y, zc);
+                        fma2_bcast(acc[p][r + 2], kv.z, zc); fma2_bcast(acc[p][r + 3], kv.w, zc);
                     }
                 }
             }
