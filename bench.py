@@ -125,6 +125,47 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_dump(args, ctx, w, x0s, ticks, stream, info):
+    """a9: trajectory-dump path. Every launch writes H*J*N fp32 (NaN after a candidate's first
+    violating state), candidate fastest; bounded by HBM write bandwidth where 2d(d+m)/(4J) flop/B is
+    below the machine balance (lifted dumps at d = 8, 16), by the FP32 pipe otherwise."""
+    import torch
+    import paper_1906_02318_b200 as mp
+    N, H = w.N, w.H
+    J = w.d if args.dump == "lifted" else w.n
+    kind = mp.DUMP_LIFTED if args.dump == "lifted" else mp.DUMP_PHYS
+    traj = torch.empty((H, J, N), dtype=torch.float32, device="cuda")
+    steps = torch.empty(N, dtype=torch.int32, device="cuda")
+    dX0 = torch.as_tensor(x0s).cuda().contiguous()
+    K_, W_ = args.steps, args.warmup
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K_)]
+    for t in range(W_ + K_):
+        if t >= W_:
+            ev[t - W_][0].record()
+        ctx.rollout_batch(0, dX0[t].data_ptr(), 1, N, H, kind, traj.data_ptr(), steps.data_ptr(), 0, int(ticks[t]), stream)
+        if t >= W_:
+            ev[t - W_][1].record()
+    torch.cuda.synchronize()
+    ms = np.array([a.elapsed_time(b) for a, b in ev])
+    nbytes = float(N) * H * J * 4 + 4.0 * N
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    gbs = nbytes / (ms.mean() * 1e-3) / 1e9
+    n_exec = int(torch.clamp(steps.to(torch.int64) + 1, max=H).sum().item())
+    flop_b = _flop_per_sample_step(w) / (4.0 * J)
+    print(json.dumps({
+        "metric": "trajectory dump bandwidth", "value": gbs, "unit": "GB/s", "n_gpus": 1, "steps": K_, "warmup": W_,
+        "ms_per_step": float(ms.mean()), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"{args.workload} dump={args.dump}: d={w.d} J={J} N={N} H={H}; output {nbytes / 1e9:.2f} GB per launch "
+                               "(larger than L2, so no flush is needed)", "kernel": info},
+        "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                     "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy; of measured)" if peaks else "fallback 6650 GB/s",
+                     "flop_per_byte": flop_b, "machine_balance_flop_per_byte": FP32_PEAK_TFLOPS * 1e3 / peak,
+                     "fp32_frac_nominal": float(N) * H * _flop_per_sample_step(w) / (ms.mean() * 1e-3) / 1e12 / FP32_PEAK_TFLOPS},
+        "executed_sample_steps": n_exec, "gpu_launches": K_}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -135,6 +176,10 @@ def main():
     ap.add_argument("--N", type=int, default=None, help="override candidates per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-latency", action="store_true")
+    ap.add_argument("--dump", choices=["lifted", "phys"], default=None,
+                    help="measure the trajectory-dump path (mpmi_rollout_batch, SURVEY 8(a) a9) instead of the tick")
+    ap.add_argument("--bounds-scale", type=float, default=1.0,
+                    help="scale the safe set (100 = every rollout safe: no early exit, full N*H work)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
@@ -160,6 +205,8 @@ def main():
     w1 = W.make(args.workload, N=args.N)
     n_per = w1.N
     w = W.make(args.workload, N=n_per * world)
+    if args.bounds_scale != 1.0:
+        w = W.generate.scaled_bounds(w, args.bounds_scale)
     K_, W_ = args.steps, args.warmup
     x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
@@ -167,6 +214,8 @@ def main():
     ctx = mp.Context(w, device=local, shard=(begin, count) if world > 1 else (0, 0))
     info = ctx.info()
     stream = torch.cuda.current_stream().cuda_stream
+    if args.dump:
+        return run_dump(args, ctx, w, x0s, ticks, stream, info)
 
     dX0 = torch.as_tensor(x0s).cuda().contiguous()
     dUU = torch.as_tensor(uus).cuda().contiguous()
@@ -292,7 +341,8 @@ def main():
         "steps": K_, "warmup": W_, "ms_per_step": total_ms / K_, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{args.workload}: n={w.n} m={w.m} d={w.d} N={n_per}/GPU (+1 user slot) H={w.H}, "
-                               f"Philox/grid sampler, calibrated 40% safe (DESIGN.md section 4)",
+                               f"Philox/grid sampler, calibrated 40% safe (DESIGN.md section 4)"
+                               + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else ""),
                    "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
                    "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if world > 1 else "single GPU",
                    "kernel": info},

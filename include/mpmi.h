@@ -55,7 +55,10 @@ enum { MPMI_DUMP_NONE = 0, MPMI_DUMP_PHYS = 1, MPMI_DUMP_LIFTED = 2 };
 enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)                  */
        MPMI_VARIANT_WIDE = 2,           /* 64/D candidates per thread (throughput)            */
        MPMI_VARIANT_NO_BINNING = 4,     /* never order the Philox candidates spatially        */
-       MPMI_VARIANT_FORCE_BINNING = 8 };/* order them even for small N                        */
+       MPMI_VARIANT_FORCE_BINNING = 8,  /* order them even for small N                        */
+       MPMI_VARIANT_LATENCY = 16,       /* several lanes per candidate (d <= 32), any N       */
+       MPMI_VARIANT_LAT_R2 = 32,        /* latency kernel: 2 rows per lane                    */
+       MPMI_VARIANT_LAT_R4 = 64 };      /* latency kernel: 4 rows per lane                    */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:
@@ -127,7 +130,8 @@ typedef struct {
 
 typedef struct {
     int32_t  d_pad;           /* internal padded lifted dim (zero rows / columns: exact)            */
-    int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = CTA-tile FFMA2 (d<=128)   */
+    int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = warp-tile FFMA2 (d<=128),
+                                 3 = latency kernel, 4 lanes per candidate (d<=32, small N)          */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;
     int32_t  binning_cells;   /* 0 = candidates walked in index order; else cells of the spatial pre-sort */

@@ -15,7 +15,6 @@
 namespace mpmi {
 
 struct BinArgs {
-    const unsigned long long *tick_ptr;
     unsigned long long tick_val;
     long long nsamp;          // sampled candidates of this shard (the injected u_h is not binned)
     int bits[kMaxM];          // cell bits per input dimension
@@ -38,7 +37,7 @@ __device__ __forceinline__ int cell_of(const DevCfg &cfg, const BinArgs &b, long
 }
 
 __global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
-    const unsigned long long tick = b.tick_ptr ? *b.tick_ptr : b.tick_val;
+    const unsigned long long tick = b.tick_val;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < b.nsamp; i += (long long)gridDim.x * blockDim.x)
         atomicAdd(&b.hist[cell_of(cfg, b, cfg.shard_begin + i, tick)], 1);
     __shared__ bool last;
@@ -87,7 +86,7 @@ __global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ D
 }
 
 __global__ void __launch_bounds__(256) bin_scatter_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
-    const unsigned long long tick = b.tick_ptr ? *b.tick_ptr : b.tick_val;
+    const unsigned long long tick = b.tick_val;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < b.nsamp; i += (long long)gridDim.x * blockDim.x) {
         const int pos = atomicAdd(&b.cursor[cell_of(cfg, b, cfg.shard_begin + i, tick)], 1);
         b.perm[pos] = (int)i;

@@ -10,8 +10,12 @@ struct KArgs {
     // tick
     const float *x0;                      // device, n   (MODE_TICK; MODE_BATCH with x0_count == 1)
     const float *u_user;                  // device, m
-    const unsigned long long *tick_ptr;   // device or null -> tick_val
     unsigned long long tick_val;
+    // host path: the tick inputs travel BY VALUE inside the kernel-node parameters (no H2D copy node)
+    float x0_val[kMaxN];
+    float u_val[kMaxM];
+    int inline_inputs;                    // 1: read x0_val / u_val instead of x0 / u_user
+    unsigned seq;                         // written last into out->reserved (host polls it on mapped memory)
     TickState *st;
     mpmi_result *out;
     mpmi_partial *partial;

@@ -3,6 +3,7 @@
 // choice, the per-tick CUDA graph (param H2D -> fused tick kernel -> result D2H),
 // pinned staging, and the benchmark entry mpmi_rollout_batch.  No CPU fallback: every step of the
 // path runs in the kernels of rollout_reg.cuh / rollout_tile.cuh.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -21,16 +22,24 @@ using namespace mpmi;
 struct mpmi_ctx {
     DevCfg dc;
     int device = 0, sm_count = 0;
-    int variant = 0, P = 1, block = 128, cand_per_block = 0, smem = 0, regs = 0;
+    int variant = 0, P = 1, smem = 0, regs = 0;
+    int block = 128, cand_per_block = 0;              // launch geometry of the tick kernel
+    int bblock = 128, bcand_per_block = 0;            // launch geometry of the batch kernel
     KernFn k_tick = nullptr, k_batch = nullptr;
     float *d_KTa = nullptr, *d_W = nullptr, *d_b = nullptr;
     uint8_t *d_terms = nullptr;
-    TickIn *d_in = nullptr, *h_in = nullptr;
     TickState *d_state = nullptr;
-    mpmi_result *d_res = nullptr, *h_res = nullptr;
+    mpmi_result *h_res = nullptr, *d_res_mapped = nullptr;   // pinned + mapped: the tick kernel writes the result here
+    // the tick as ONE CUDA graph: [cell histogram, scatter,] fused tick kernel.  The tick inputs travel
+    // inside the kernel-node parameters (updated per launch), the result comes back through mapped memory.
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
-    cudaEvent_t done = nullptr;
+    cudaGraphNode_t n_hist = nullptr, n_scatter = nullptr, n_tick = nullptr;
+    unsigned bin_grid = 0, tick_grid = 0;
+    KArgs ga{};
+    BinArgs gb{};
+    unsigned seq = 0;
+    cudaStream_t pending_stream = nullptr;
     bool pending = false;
     // spatial binning of Philox candidates (binning.cuh)
     bool binning = false;
@@ -59,6 +68,8 @@ __global__ void shard_finalise_kernel(const __grid_constant__ DevCfg cfg, const 
 
 namespace {
 
+constexpr long long kLatMaxCand = 1 << 15;      // <= this many candidates: latency kernel (measured crossover)
+
 thread_local std::string g_create_err;
 
 #define CU(ctx, call)                                                                      \
@@ -81,6 +92,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 #define MPMI_DECL_TILE(D) KernFn mpmi_pick_tile_##D##_tick(int M, int *smem); KernFn mpmi_pick_tile_##D##_batch(int M, int *smem);
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
+KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
 KernFn pick_reg(int D, int M, int P, int mode) {
     const bool t = mode == MODE_TICK;
@@ -90,6 +102,9 @@ KernFn pick_reg(int D, int M, int P, int mode) {
         case 32: return t ? mpmi_pick_reg_32_tick(M, P) : mpmi_pick_reg_32_batch(M, P);
     }
     return nullptr;
+}
+KernFn pick_lat(int D, int M, int R) {
+    return D == 8 ? mpmi_pick_lat_8(M, R) : D == 16 ? mpmi_pick_lat_16(M, R) : D == 32 ? mpmi_pick_lat_32(M, R) : nullptr;
 }
 KernFn pick_tile(int D, int M, int mode, int *smem) {
     const bool t = mode == MODE_TICK;
@@ -104,7 +119,9 @@ bool all_finite(const float *p, size_t n) {
 }
 
 void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
-    long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
+    const bool batch = fn == c->k_batch;
+    const int cpb = batch ? c->bcand_per_block : c->cand_per_block, block = batch ? c->bblock : c->block;
+    long long blocks = (ncand + cpb - 1) / cpb;
     if (blocks < 1) blocks = 1;
     KArgs a = a0;
     if (c->variant == 2) {                       // persistent warp-tile kernel: one CTA per SM
@@ -112,14 +129,14 @@ void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cuda
         a.st = c->d_state; a.work = &c->d_state->work;
     }
     void *args[2] = {(void *)&c->dc, (void *)&a};
-    cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)c->block), args, (size_t)c->smem, s);
+    cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)c->smem, s);
 }
 
 // one tick on stream s: [cell histogram + scan, scatter] (large Philox sets only) -> fused tick kernel
 void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
     if (c->binning) {
         BinArgs b = c->bin;
-        b.tick_ptr = a.tick_ptr; b.tick_val = a.tick_val;
+        b.tick_val = a.tick_val;
         long long g = (b.nsamp + 255) / 256;
         const long long gmax = 8LL * c->sm_count;
         const unsigned grid = (unsigned)(g < gmax ? g : gmax);
@@ -130,19 +147,49 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
     launch(c, c->k_tick, c->dc.shard_count, a, s);
 }
 
+unsigned grid_for(const mpmi_ctx *c, long long ncand) {
+    long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
+    if (blocks < 1) blocks = 1;
+    if (c->variant == 2 && blocks > c->sm_count) blocks = c->sm_count;
+    return (unsigned)blocks;
+}
+
+void tick_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
+    p->func = (void *)c->k_tick; p->gridDim = dim3(c->tick_grid); p->blockDim = dim3((unsigned)c->block);
+    p->sharedMemBytes = (unsigned)c->smem; p->kernelParams = args;
+}
+void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **args) {
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->gb;
+    p->func = scatter ? (void *)bin_scatter_kernel : (void *)bin_hist_kernel;
+    p->gridDim = dim3(c->bin_grid); p->blockDim = dim3(256); p->kernelParams = args;
+}
+
 int build_graph(mpmi_ctx *c) {
-    cudaStream_t s;
-    CU(c, cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
-    KArgs a{};
-    a.x0 = c->d_in->x0; a.u_user = c->d_in->u_user; a.tick_ptr = &c->d_in->tick;
-    a.st = c->d_state; a.out = c->d_res;
-    CU(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
-    cudaMemcpyAsync(c->d_in, c->h_in, sizeof(TickIn), cudaMemcpyHostToDevice, s);
-    enqueue_tick(c, a, s);
-    cudaMemcpyAsync(c->h_res, c->d_res, sizeof(mpmi_result), cudaMemcpyDeviceToHost, s);
-    CU(c, cudaStreamEndCapture(s, &c->graph));
+    c->ga = KArgs{};
+    c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1;
+    if (c->variant == 2) c->ga.work = &c->d_state->work;
+    c->tick_grid = grid_for(c, c->dc.shard_count);
+    CU(c, cudaGraphCreate(&c->graph, 0));
+    cudaKernelNodeParams p; void *args[2];
+    cudaGraphNode_t dep = nullptr;
+    if (c->binning) {
+        c->gb = c->bin;
+        long long g = (c->gb.nsamp + 255) / 256;
+        const long long gmax = 8LL * c->sm_count;
+        c->bin_grid = (unsigned)(g < gmax ? g : gmax);
+        c->ga.perm = c->d_perm; c->ga.nsamp = c->gb.nsamp;
+        bin_node_params(c, false, &p, args);
+        CU(c, cudaGraphAddKernelNode(&c->n_hist, c->graph, nullptr, 0, &p));
+        bin_node_params(c, true, &p, args);
+        CU(c, cudaGraphAddKernelNode(&c->n_scatter, c->graph, &c->n_hist, 1, &p));
+        dep = c->n_scatter;
+    }
+    tick_node_params(c, &p, args);
+    CU(c, cudaGraphAddKernelNode(&c->n_tick, c->graph, dep ? &dep : nullptr, dep ? 1 : 0, &p));
     CU(c, cudaGraphInstantiate(&c->exec, c->graph, 0));
-    CU(c, cudaStreamDestroy(s));
     return MPMI_OK;
 }
 
@@ -166,13 +213,13 @@ const char *mpmi_last_error(const mpmi_ctx *ctx) { return ctx ? ctx->err.c_str()
 void mpmi_destroy(mpmi_ctx *c) {
     if (!c) return;
     cudaSetDevice(c->device);
-    if (c->done) { cudaEventSynchronize(c->done); cudaEventDestroy(c->done); }
+    if (c->pending) cudaStreamSynchronize(c->pending_stream);
     if (c->exec) cudaGraphExecDestroy(c->exec);
     if (c->graph) cudaGraphDestroy(c->graph);
     cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
-    cudaFree(c->d_in); cudaFree(c->d_state); cudaFree(c->d_res);
+    cudaFree(c->d_state);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
-    cudaFreeHost(c->h_in); cudaFreeHost(c->h_res);
+    cudaFreeHost(c->h_res);
     delete c;
 }
 
@@ -314,16 +361,12 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         CUC(cudaMemcpy(c->d_b, L.b, (size_t)(d - n) * sizeof(float), cudaMemcpyHostToDevice));
     }
     dc.KTa = c->d_KTa; dc.terms = c->d_terms; dc.W = c->d_W; dc.b = c->d_b;
-    CUC(cudaMalloc(&c->d_in, sizeof(TickIn)));
-    CUC(cudaMemset(c->d_in, 0, sizeof(TickIn)));
     CUC(cudaMalloc(&c->d_state, sizeof(TickState)));
     TickState st0{kKeyNone, 0ull, 0u, 0u, 0u, 0u};
     CUC(cudaMemcpy(c->d_state, &st0, sizeof st0, cudaMemcpyHostToDevice));
-    CUC(cudaMalloc(&c->d_res, sizeof(mpmi_result)));
-    CUC(cudaHostAlloc(&c->h_in, sizeof(TickIn), cudaHostAllocDefault));
-    CUC(cudaHostAlloc(&c->h_res, sizeof(mpmi_result), cudaHostAllocDefault));
-    std::memset(c->h_in, 0, sizeof(TickIn));
-    CUC(cudaEventCreateWithFlags(&c->done, cudaEventDisableTiming));
+    CUC(cudaHostAlloc(&c->h_res, sizeof(mpmi_result), cudaHostAllocMapped));
+    std::memset(c->h_res, 0, sizeof(mpmi_result));
+    CUC(cudaHostGetDevicePointer((void **)&c->d_res_mapped, c->h_res, 0));
 
     // ---- spatial binning: large Philox candidate sets only (the grid is already spatially ordered)
     {
@@ -358,12 +401,25 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         const long long threads = (sc + 2LL * c->P - 1) / (2LL * c->P);
         c->block = threads >= 128LL * 2 * c->sm_count ? 128 : threads >= 64LL * 2 * c->sm_count ? 64 : 32;
         c->cand_per_block = 2 * c->P * c->block;
+        c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
         c->smem = 0;
         c->k_tick = pick_reg(D, M, c->P, MODE_TICK);
         c->k_batch = pick_reg(D, M, c->P, MODE_BATCH);
+        // paper-scale candidate sets: 4 lanes per candidate (rollout_lat.cuh) shorten the dependent chain
+        const bool lat = (cfg->variant & MPMI_VARIANT_LATENCY) || (!(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE)) && sc <= kLatMaxCand);
+        if (lat && !c->binning) {
+            // rows per lane: 2 (D/2 lanes per candidate) while that still leaves SMs short of warps, else 4
+            const long long warps_r4 = sc * (D / 4) / 32;
+            const int R = (cfg->variant & MPMI_VARIANT_LAT_R2) ? 2 : (cfg->variant & MPMI_VARIANT_LAT_R4) ? 4
+                          : (warps_r4 < 24LL * c->sm_count ? 2 : 4);
+            c->variant = 3;
+            c->k_tick = pick_lat(D, M, R);
+            c->block = 64; c->cand_per_block = 64 / (D / R);     // D/R lanes per candidate
+        }
     } else {
         c->variant = 2;
         c->P = 1; c->block = kTileThreads; c->cand_per_block = kTileNC;
+        c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
         c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem);
         c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem);
         if (c->k_tick) {
@@ -401,13 +457,28 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     if (!x0 || !u_user) return fail(c, MPMI_ERR_INVALID, "null x0 or u_user");
     if (!all_finite(x0, c->dc.n) || !all_finite(u_user, c->dc.m)) return fail(c, MPMI_ERR_INVALID, "non-finite x0 or u_user");
     CU(c, cudaSetDevice(c->device));
-    if (c->pending) { CU(c, cudaEventSynchronize(c->done)); c->pending = false; }   // one tick in flight
-    std::memcpy(c->h_in->x0, x0, sizeof(float) * c->dc.n);
-    std::memcpy(c->h_in->u_user, u_user, sizeof(float) * c->dc.m);
-    c->h_in->tick = tick;
+    if (c->pending) {                                       // one tick in flight per context
+        mpmi_result drop;
+        const int rc = mpmi_step_result(c, &drop);
+        if (rc != MPMI_OK) return rc;
+    }
+    std::memcpy(c->ga.x0_val, x0, sizeof(float) * c->dc.n);
+    std::memcpy(c->ga.u_val, u_user, sizeof(float) * c->dc.m);
+    c->ga.tick_val = tick;
+    if (++c->seq == 0) c->seq = 1;
+    c->ga.seq = c->seq;
+    cudaKernelNodeParams p; void *args[2];
+    if (c->binning) {
+        c->gb.tick_val = tick;
+        bin_node_params(c, false, &p, args);
+        CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_hist, &p));
+        bin_node_params(c, true, &p, args);
+        CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_scatter, &p));
+    }
+    tick_node_params(c, &p, args);
+    CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_tick, &p));
     CU(c, cudaGraphLaunch(c->exec, (cudaStream_t)stream));
-    CU(c, cudaEventRecord(c->done, (cudaStream_t)stream));
-    c->pending = true;
+    c->pending = true; c->pending_stream = (cudaStream_t)stream;
     c->err.clear();
     return MPMI_OK;
 }
@@ -415,9 +486,21 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
 int mpmi_step_result(mpmi_ctx *c, mpmi_result *out) {
     if (!c || !out) return MPMI_ERR_INVALID;
     if (!c->pending) return fail(c, MPMI_ERR_INVALID, "no tick in flight");
-    CU(c, cudaEventSynchronize(c->done));
+    // the last CTA of the tick kernel writes the result into mapped pinned memory and then its sequence
+    // number; poll for it (cheaper than a stream synchronise), checking the stream for errors now and then
+    volatile mpmi_result *h = c->h_res;
+    const int want = (int)c->seq;
+    for (unsigned spin = 0; h->reserved != want; spin++) {
+        if ((spin & 0x3FFF) == 0x3FFF) {
+            const cudaError_t e = cudaStreamQuery(c->pending_stream);
+            if (e == cudaSuccess) { if (h->reserved != want) { c->pending = false; return fail(c, MPMI_ERR_CUDA, "tick finished without a result"); } break; }
+            if (e != cudaErrorNotReady) { c->pending = false; c->err = std::string("tick failed: ") + cudaGetErrorString(e); return MPMI_ERR_CUDA; }
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
     c->pending = false;
-    *out = *c->h_res;
+    std::memcpy(out, c->h_res, sizeof *out);
+    out->reserved = 0;
     return MPMI_OK;
 }
 
@@ -432,7 +515,7 @@ int mpmi_step_device(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint
     if (!d_x0 || !d_u_user || !d_out) return fail(c, MPMI_ERR_INVALID, "null device pointer");
     CU(c, cudaSetDevice(c->device));
     KArgs a{};
-    a.x0 = d_x0; a.u_user = d_u_user; a.tick_ptr = nullptr; a.tick_val = tick;
+    a.x0 = d_x0; a.u_user = d_u_user; a.tick_val = tick;
     a.st = c->d_state; a.out = d_out;
     enqueue_tick(c, a, (cudaStream_t)stream);
     CU(c, cudaGetLastError());
@@ -444,7 +527,7 @@ int mpmi_shard_step(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint6
     if (!d_x0 || !d_u_user || !d_partial) return fail(c, MPMI_ERR_INVALID, "null device pointer");
     CU(c, cudaSetDevice(c->device));
     KArgs a{};
-    a.x0 = d_x0; a.u_user = d_u_user; a.tick_ptr = nullptr; a.tick_val = tick;
+    a.x0 = d_x0; a.u_user = d_u_user; a.tick_val = tick;
     a.st = c->d_state; a.out = nullptr; a.partial = d_partial;
     enqueue_tick(c, a, (cudaStream_t)stream);
     CU(c, cudaGetLastError());
@@ -471,7 +554,7 @@ int mpmi_rollout_batch(mpmi_ctx *c, const float *d_U, const float *d_X0, int64_t
         return fail(c, MPMI_ERR_INVALID, "bad dump_kind or null d_traj");
     CU(c, cudaSetDevice(c->device));
     KArgs a{};
-    a.x0 = d_X0; a.u_user = nullptr; a.tick_ptr = nullptr; a.tick_val = tick;
+    a.x0 = d_X0; a.u_user = nullptr; a.tick_val = tick;
     a.U = d_U; a.x0_count = x0_count; a.ncand = Ncand; a.H = H; a.dump_kind = dump_kind;
     a.traj = d_traj; a.steps = d_steps; a.safe = d_safe;
     launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream);

@@ -36,14 +36,6 @@ struct DevCfg {
     const float *W, *b;             // device: RFF tables
 };
 
-// Inputs of one tick as they sit in device memory.
-struct TickIn {
-    float x0[kMaxN];
-    float u_user[kMaxM];
-    unsigned long long tick;
-    unsigned long long pad;
-};
-
 // Cross-block selection state; reset by the block that finalises the tick.
 struct TickState {
     unsigned long long best_key;
@@ -188,7 +180,7 @@ __device__ __forceinline__ unsigned warp_sum_u32(unsigned v) {
 // If `partial` is non-null the block writes the shard's mpmi_partial instead (multi-GPU path).
 __device__ __forceinline__ void decode_result(const DevCfg &cfg, unsigned long long key, unsigned long long n_exec,
                                               unsigned n_safe, unsigned long long tick,
-                                              const float (&u_h)[kMaxM], mpmi_result *out) {
+                                              const float (&u_h)[kMaxM], mpmi_result *out, unsigned seq = 0) {
     mpmi_result r;
     const long long gi = (long long)(key & ((1ull << kKeyIndexBits) - 1));
     const bool safe = ((key >> 62) & 1ull) == 0;
@@ -212,6 +204,10 @@ __device__ __forceinline__ void decode_result(const DevCfg &cfg, unsigned long l
     r.key = key;
     if (key == kKeyNone) { r.index = -1; r.safe = 0; r.steps = 0; r.dist = 0.0f; }
     *out = r;
+    if (seq) {                       // out is host-mapped: publish the sequence number after the payload
+        __threadfence_system();
+        *reinterpret_cast<volatile int *>(&out->reserved) = (int)seq;
+    }
 }
 
 template <int kWarps>
@@ -219,7 +215,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                                                           unsigned n_safe, unsigned long long n_exec,
                                                           unsigned long long tick, const float (&u_h)[kMaxM],
                                                           TickState *st, mpmi_result *out, mpmi_partial *partial,
-                                                          unsigned *work = nullptr) {
+                                                          unsigned seq = 0, unsigned *work = nullptr) {
     __shared__ unsigned long long s_key[kWarps];
     __shared__ unsigned s_safe[kWarps];
     __shared__ unsigned long long s_exec[kWarps];
@@ -252,7 +248,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
             if (partial) {
                 partial->key = bk; partial->n_safe = tot_safe; partial->n_exec = (long long)tot_exec;
             } else {
-                decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out);
+                decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out, seq);
             }
             st->best_key = kKeyNone; st->n_exec = 0ull; st->n_safe = 0u; st->ticket = 0u;   // ready for next tick
             if (work) *work = 0u;
@@ -275,6 +271,15 @@ __device__ __forceinline__ void fma2_bcast(float2 &acc, float k, const float2 &z
     unsigned long long kk, zz, aa;
     asm("mov.b64 %0, {%1,%1};" : "=l"(kk) : "f"(k));
     asm("mov.b64 %0, {%1,%2};" : "=l"(zz) : "f"(z.x), "f"(z.y));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(aa) : "f"(acc.x), "f"(acc.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(aa) : "l"(kk), "l"(zz));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
+}
+// acc += kpair * z on a ROW pair of one candidate: the state value is the broadcast operand
+__device__ __forceinline__ void fma2_bcast_z(float2 &acc, const float2 &k, float z) {
+    unsigned long long kk, zz, aa;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(kk) : "f"(k.x), "f"(k.y));
+    asm("mov.b64 %0, {%1,%1};" : "=l"(zz) : "f"(z));
     asm("mov.b64 %0, {%1,%2};" : "=l"(aa) : "f"(acc.x), "f"(acc.y));
     asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(aa) : "l"(kk), "l"(zz));
     asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));

@@ -58,7 +58,9 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     const int tid = threadIdx.x, bdim = blockDim.x;
     for (int i = tid; i < (D + M) * D / 4; i += bdim)
         reinterpret_cast<float4 *>(sK)[i] = reinterpret_cast<const float4 *>(cfg.KTa)[i];
-    const unsigned long long tick = a.tick_ptr ? *a.tick_ptr : a.tick_val;
+    const unsigned long long tick = a.tick_val;
+    const float *x0p = a.inline_inputs ? a.x0_val : a.x0;
+    const float *uup = a.inline_inputs ? a.u_val : a.u_user;
     const int H = (MODE == MODE_TICK) ? cfg.H : a.H;
     const long long ncand = (MODE == MODE_TICK) ? cfg.shard_count : a.ncand;
     const bool shared_x0 = (MODE == MODE_TICK) || a.x0_count == 1;
@@ -66,11 +68,11 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     float u_h[kMaxM] = {0.f, 0.f, 0.f, 0.f};
     bool inputs_ok = true;
     if (MODE == MODE_TICK) {
-        inputs_ok = finite_inputs(cfg, a.x0, a.u_user);
-        clamp_user(cfg, a.u_user, u_h);
+        inputs_ok = finite_inputs(cfg, x0p, uup);
+        clamp_user(cfg, uup, u_h);
     }
     if (shared_x0) {
-        for (int f = tid; f < D; f += bdim) sz0[f] = lift_feature(cfg, f, a.x0);
+        for (int f = tid; f < D; f += bdim) sz0[f] = lift_feature(cfg, f, x0p);
     }
     __syncthreads();
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(sK);
@@ -218,7 +220,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
             n_exec += (unsigned)(steps[s] + 1 < H ? steps[s] + 1 : H);
         }
     }
-    block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial);
+    block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq);
 }
 
 }  // namespace mpmi
