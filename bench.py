@@ -64,7 +64,7 @@ class ClockSampler(threading.Thread):
                 self.samples.append((sm, mx, rs))
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.004)
 
     def summary(self):
         if not self.samples:
@@ -278,7 +278,9 @@ def main():
             wall.append(time.perf_counter() - t0)
             e_exec += rr.n_exec
         t_all = time.perf_counter() - t_all
-        e2e = {"value": e_exec / t_all, "unit": "sample-steps/s", "h2d_bytes_per_step": 112, "d2h_bytes_per_step": 56,
+        e2e = {"value": e_exec / t_all, "unit": "sample-steps/s", "h2d_bytes_per_step": 4 * (w.n + w.m) + 8, "d2h_bytes_per_step": 56,
+               "transport": "x0, u_user, tick ride in the graph's kernel-node parameters; the 56-byte result is written "
+                            "by the kernel into mapped pinned host memory and polled",
                "ms_per_step": 1e3 * t_all / K_}
         p50, p99 = _percentiles(wall)
         lat[f"{args.workload}_N{w.N}"] = {"host_p50_us": 1e6 * p50, "host_p99_us": 1e6 * p99,
@@ -348,7 +350,7 @@ def main():
                    "kernel": info},
         "nominal_value": nominal / (total_ms * 1e-3), "executed_fraction": n_exec / nominal,
         "safe_fraction": float(res["n_safe"][W_:].mean() / (w.N + 1)),
-        "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": K_ * (1 if world == 1 else 2),
+        "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": K_ * (info["launches_per_tick"] + (1 if world > 1 else 0)),
         "roofline": roofline, "cpu_baseline": cpu, "latency": lat,
         "paper_context": "paper: >10,000 trajectories per tick at ~100 Hz / ~60 Hz on a GeForce 860M (PAPER.md:12, 266)",
     }

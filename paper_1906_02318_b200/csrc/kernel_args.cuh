@@ -35,8 +35,8 @@ struct KArgs {
 
 enum { MODE_TICK = 0, MODE_BATCH = 1 };
 
-constexpr int kTileThreads = 256;
-constexpr int kTileNC = 256;
+constexpr int kTileNC = 256;                      // candidates per CTA pass of the warp-tile kernel
+constexpr int kTileThreads = 512;                 // = (kTileNC / 16 candidates per warp) * 32
 
 }  // namespace mpmi
 

@@ -411,7 +411,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             // rows per lane: 2 (D/2 lanes per candidate) while that still leaves SMs short of warps, else 4
             const long long warps_r4 = sc * (D / 4) / 32;
             const int R = (cfg->variant & MPMI_VARIANT_LAT_R2) ? 2 : (cfg->variant & MPMI_VARIANT_LAT_R4) ? 4
-                          : (warps_r4 < 24LL * c->sm_count ? 2 : 4);
+                          : (warps_r4 < 4LL * c->sm_count ? 2 : 4);
             c->variant = 3;
             c->k_tick = pick_lat(D, M, R);
             c->block = 64; c->cand_per_block = 64 / (D / R);     // D/R lanes per candidate

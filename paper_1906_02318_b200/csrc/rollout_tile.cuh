@@ -18,18 +18,23 @@
 
 namespace mpmi {
 
-constexpr int kTileWC = 32;                      // candidates per warp batch
-constexpr int kTileWarps = kTileThreads / 32;
+constexpr int kTileWC = 16;                      // candidates per warp batch (16 -> 16 warps per CTA)
+constexpr int kTileWarps = kTileNC / kTileWC;
+constexpr int kTileThreadsT = kTileWarps * 32;
 
 template <int D, int M>
 constexpr int tile_smem_bytes() { return ((D + M) * D + kTileWarps * (D + M) * kTileWC) * 4; }
 
 template <int D, int M, int MODE>
-__global__ void __launch_bounds__(kTileThreads, 1)
+__global__ void __launch_bounds__(kTileThreadsT, 1)
 rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     constexpr int WC = kTileWC;
-    constexpr int TR = D / 8;                     // rows per lane (8 row groups x 4 candidate groups)
+    constexpr int CG = WC / 8;                    // candidate groups per warp: every lane owns 8 candidates
+    constexpr int RG = 32 / CG;                   // row groups per warp
+    constexpr int TR = D / RG;                    // rows per lane
     constexpr int QR = TR / 4;                    // float4 groups of rows per lane
+    constexpr int kTileThreads = kTileThreadsT;
+    static_assert(TR % 4 == 0, "lane tile");
     static_assert(D == 64 || D == 128, "tile kernel: D in {64, 128}");
     extern __shared__ __align__(16) float smem[];
     float *sK = smem;                             // (D+M) x D
@@ -63,9 +68,10 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
     const int nphys = cfg.annulus ? (nbox > 2 ? nbox : 2) : nbox;      // internal dims the safe test reads
     const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
     const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
-    const int rg = lane >> 2, cg = lane & 3;
-    const float *kp = sK + rg * 4;                // rows  q*32 + rg*4 + e,  q < QR
-    const float *zp = zw + cg * 4;                // cands q*16 + cg*4 + e,  q < 2
+    const int rg = lane / CG, cg = lane % CG;
+    const float *kp = sK + rg * 4;                // rows  q*(4 RG) + rg*4 + e,  q < QR
+    const float *zp = zw + cg * 4;                // cands q*(4 CG) + cg*4 + e,  q < 2
+    const int col = lane % WC;                    // the candidate this lane fills and tests (lanes >= WC mirror)
     const long long nbatch = (ncand + WC - 1) / WC;
 
     unsigned long long key = kKeyNone;
@@ -80,7 +86,7 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
         if (batch >= nbatch) break;
 
         // ---- a1 + a2: lane i fills column i of the warp tile
-        long long li = batch * WC + lane;
+        long long li = batch * WC + col;
         if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];   // spatially ordered walk
         bool alive = li < ncand && inputs_ok;
         int steps = 0;
@@ -94,14 +100,14 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
                 }
             }
 #pragma unroll
-            for (int j = 0; j < M; j++) zw[(D + j) * WC + lane] = u[j];
+            for (int j = 0; j < M; j++) zw[(D + j) * WC + col] = u[j];
             if (shared_x0) {
-                for (int c = 0; c < D; c++) zw[c * WC + lane] = sz0[c];
+                for (int c = 0; c < D; c++) zw[c * WC + col] = sz0[c];
             } else {
                 float x[kMaxN];
                 const long long row = li < ncand ? li : 0;
                 for (int j = 0; j < kMaxN; j++) x[j] = j < cfg.n ? a.x0[row * cfg.n + j] : 0.f;
-                for (int c = 0; c < D; c++) zw[c * WC + lane] = lift_feature(cfg, c, x);
+                for (int c = 0; c < D; c++) zw[c * WC + col] = lift_feature(cfg, c, x);
             }
         }
         __syncwarp();
@@ -122,13 +128,13 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
                 float kr[TR];
 #pragma unroll
                 for (int q = 0; q < QR; q++) {
-                    const float4 v = *reinterpret_cast<const float4 *>(kp + c * D + q * 32);
+                    const float4 v = *reinterpret_cast<const float4 *>(kp + c * D + q * (4 * RG));
                     kr[4 * q] = v.x; kr[4 * q + 1] = v.y; kr[4 * q + 2] = v.z; kr[4 * q + 3] = v.w;
                 }
                 float2 zc[4];
 #pragma unroll
                 for (int q = 0; q < 2; q++) {
-                    const float4 v = *reinterpret_cast<const float4 *>(zp + c * WC + q * 16);
+                    const float4 v = *reinterpret_cast<const float4 *>(zp + c * WC + q * (4 * CG));
                     zc[2 * q] = make_float2(v.x, v.y);
                     zc[2 * q + 1] = make_float2(v.z, v.w);
                 }
@@ -140,46 +146,46 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
             __syncwarp();                                  // every lane has finished reading Zw
 #pragma unroll
             for (int r = 0; r < TR; r++) {
-                const int row = (r >> 2) * 32 + rg * 4 + (r & 3);
+                const int row = (r >> 2) * (4 * RG) + rg * 4 + (r & 3);
 #pragma unroll
                 for (int q = 0; q < 2; q++)
-                    *reinterpret_cast<float4 *>(zw + row * WC + q * 16 + cg * 4) =
+                    *reinterpret_cast<float4 *>(zw + row * WC + q * (4 * CG) + cg * 4) =
                         make_float4(acc[r][2 * q].x, acc[r][2 * q].y, acc[r][2 * q + 1].x, acc[r][2 * q + 1].y);
             }
             __syncwarp();
 
             float x[NB];
 #pragma unroll
-            for (int j = 0; j < NB; j++) x[j] = j < nphys ? zw[j * WC + lane] : 0.f;
+            for (int j = 0; j < NB; j++) x[j] = j < nphys ? zw[j * WC + col] : 0.f;
             const bool was_alive = alive;
             const bool ok = safe_check<NB>(cfg, x, nbox);
             alive = was_alive && ok;
             steps += alive ? 1 : 0;
-            if (dump && li < ncand) {
+            if (dump && li < ncand && lane < WC) {
                 for (int j = 0; j < D; j++) {
                     const int row = j < cfg.n ? (int)cfg.perm[j] : j;
                     if (row < J)
-                        a.traj[((long long)k * J + row) * ncand + li] = was_alive ? zw[j * WC + lane] : __int_as_float(0x7fc00000);
+                        a.traj[((long long)k * J + row) * ncand + li] = was_alive ? zw[j * WC + col] : __int_as_float(0x7fc00000);
                 }
             }
         }
-        if (dump && li < ncand) {
+        if (dump && li < ncand && lane < WC) {
             for (; k < H; k++)
                 for (int row = 0; row < J; row++)
                     a.traj[((long long)k * J + row) * ncand + li] = __int_as_float(0x7fc00000);
         }
 
         if (MODE == MODE_BATCH) {
-            if (li < ncand) {
+            if (li < ncand && lane < WC) {
                 a.steps[li] = steps;
                 if (a.safe) a.safe[li] = steps == H ? 1 : 0;
             }
-        } else if (li < ncand && inputs_ok) {               // a5: this candidate's key
+        } else if (li < ncand && inputs_ok && lane < WC) {  // a5: this candidate's key
             const bool safe = steps == H;
             float d2 = 0.f;
 #pragma unroll
             for (int j = 0; j < M; j++) {
-                const float df = __fsub_rn(zw[(D + j) * WC + lane], u_h[j]);
+                const float df = __fsub_rn(zw[(D + j) * WC + col], u_h[j]);
                 d2 = __fmaf_rn(df, df, d2);
             }
             const unsigned long long kk = make_key(safe, d2, H, steps, cfg.shard_begin + li);
