@@ -84,7 +84,8 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     int steps[S];
 #pragma unroll
     for (int s = 0; s < S; s++) {
-        li[s] = (long long)blockIdx.x * (S * bdim) + s * bdim + tid;
+        // the two halves of a register pair are ADJACENT candidates (2*tid, 2*tid+1): dumps store float2
+        li[s] = (long long)blockIdx.x * (S * bdim) + (s >> 1) * (2 * bdim) + 2 * tid + (s & 1);
         if (MODE == MODE_TICK && a.perm && li[s] < a.nsamp) li[s] = a.perm[li[s]];   // spatially ordered walk
         const bool valid = li[s] < ncand && inputs_ok;
         alive[s] = valid;
@@ -127,6 +128,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
     const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
     const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
+    const bool vec2 = dump && (ncand % 2 == 0) && ((reinterpret_cast<unsigned long long>(a.traj) & 7ull) == 0);
     int k = 0;
     for (; k < H; k++) {
         bool any = false;
@@ -158,23 +160,36 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
             for (int r = 0; r < D; r++) z[p][r] = acc[p][r];
 
+        bool was_alive[S];
 #pragma unroll
         for (int s = 0; s < S; s++) {
             float x[NB];
 #pragma unroll
             for (int j = 0; j < NB; j++) x[j] = (s & 1) ? z[s >> 1][j].y : z[s >> 1][j].x;
-            const bool was_alive = alive[s];
+            was_alive[s] = alive[s];
             const bool ok = safe_check<NB>(cfg, x, nbox);
-            alive[s] = was_alive && ok;
+            alive[s] = was_alive[s] && ok;
             steps[s] += alive[s] ? 1 : 0;
-            if (dump && li[s] < ncand) {
-                // a9: traj[(k*J + j)*Ncand + i], candidate fastest -> a warp writes 128 contiguous bytes
+        }
+        if (dump) {
+            // a9: traj[(k*J + j)*Ncand + i], candidate fastest.  A pair is two adjacent candidates, so one
+            // 8-byte store per (pair, row): a warp writes 256 contiguous bytes per instruction.
+            const float qnan = __int_as_float(0x7fc00000);
+            float *step_base = a.traj + (long long)k * J * ncand;
+#pragma unroll
+            for (int p = 0; p < P; p++) {
+                const long long l0 = li[2 * p];
+                const bool v0 = l0 < ncand, v1 = l0 + 1 < ncand;
 #pragma unroll
                 for (int j = 0; j < D; j++) {
                     const int row = j < cfg.n ? (int)cfg.perm[j < kMaxN ? j : 0] : j;
-                    if (row < J) {
-                        const float v = (s & 1) ? z[s >> 1][j].y : z[s >> 1][j].x;
-                        a.traj[((long long)k * J + row) * ncand + li[s]] = was_alive ? v : __int_as_float(0x7fc00000);
+                    if (row < J && v0) {
+                        float2 v = z[p][j];
+                        v.x = was_alive[2 * p] ? v.x : qnan;
+                        v.y = was_alive[2 * p + 1] ? v.y : qnan;
+                        float *q = step_base + (long long)row * ncand + l0;
+                        if (vec2 && v1) *reinterpret_cast<float2 *>(q) = v;
+                        else { q[0] = v.x; if (v1) q[1] = v.y; }
                     }
                 }
             }
