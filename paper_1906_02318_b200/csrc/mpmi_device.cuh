@@ -301,4 +301,16 @@ __device__ __forceinline__ float4 lds128(unsigned addr) {
     return v;
 }
 
+// 8-byte global store at base + 4*off (off in floats, warp-uniform): written as PTX so that the
+// address stays one IMAD.WIDE instead of being re-associated into 64-bit element arithmetic
+__device__ __forceinline__ void stg64_off(unsigned long long base, unsigned off, const float2 &v) {
+    asm volatile("{\n\t.reg .u64 a;\n\tmad.wide.u32 a, %0, 4, %1;\n\tst.global.v2.f32 [a], {%2,%3};\n\t}"
+                 :: "r"(off), "l"(base), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void stg64_off_if(unsigned long long base, unsigned off, const float2 &v, bool pred) {
+    asm volatile("{\n\t.reg .u64 a;\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\tmad.wide.u32 a, %0, 4, %1;\n\t"
+                 "@p st.global.v2.f32 [a], {%2,%3};\n\t}"
+                 :: "r"(off), "l"(base), "f"(v.x), "f"(v.y), "r"((unsigned)pred) : "memory");
+}
+
 }  // namespace mpmi

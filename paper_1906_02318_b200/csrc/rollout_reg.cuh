@@ -129,6 +129,11 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
     const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
     const bool vec2 = dump && (ncand % 2 == 0) && ((reinterpret_cast<unsigned long long>(a.traj) & 7ull) == 0);
+    const bool dump_fast = vec2 && ((long long)(blockIdx.x + 1) * (S * bdim) <= ncand) && ((long long)J * ncand < (1ll << 31));
+    const bool dump_full = J == D;           // lifted dump of an unpadded model: every row is stored
+    unsigned dump_row[NB];                   // original row of internal row j (only the first n are permuted)
+#pragma unroll
+    for (int j = 0; j < NB; j++) dump_row[j] = (dump && j < cfg.n) ? (unsigned)cfg.perm[j] : (unsigned)j;
     int k = 0;
     for (; k < H; k++) {
         bool any = false;
@@ -171,7 +176,36 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
             alive[s] = was_alive[s] && ok;
             steps[s] += alive[s] ? 1 : 0;
         }
-        if (dump) {
+        if (dump && dump_fast) {
+            // a9 fast path (whole CTA in range, aligned, one step of the dump < 2^31 floats): no per-store
+            // branches; address = per-pair pointer + warp-uniform row offset (one IMAD.WIDE per store).
+            // Row j is stored iff j < J (the internal order permutes only the first n rows among themselves).
+            const float qnan = __int_as_float(0x7fc00000);
+            const unsigned long long step_base = reinterpret_cast<unsigned long long>(a.traj + (long long)k * J * ncand);
+            const unsigned nc32 = (unsigned)ncand;
+#pragma unroll
+            for (int p = 0; p < P; p++) {
+                const unsigned long long qp = step_base + 4ull * (unsigned)li[2 * p];
+                const bool a0 = was_alive[2 * p], a1 = was_alive[2 * p + 1];
+                if (dump_full) {
+#pragma unroll
+                    for (int j = 0; j < D; j++) {
+                        float2 v = z[p][j];
+                        v.x = a0 ? v.x : qnan;
+                        v.y = a1 ? v.y : qnan;
+                        stg64_off(qp, (j < NB ? dump_row[j] : (unsigned)j) * nc32, v);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < D; j++) {
+                        float2 v = z[p][j];
+                        v.x = a0 ? v.x : qnan;
+                        v.y = a1 ? v.y : qnan;
+                        stg64_off_if(qp, (j < NB ? dump_row[j] : (unsigned)j) * nc32, v, j < J);
+                    }
+                }
+            }
+        } else if (dump) {
             // a9: traj[(k*J + j)*Ncand + i], candidate fastest.  A pair is two adjacent candidates, so one
             // 8-byte store per (pair, row): a warp writes 256 contiguous bytes per instruction.
             const float qnan = __int_as_float(0x7fc00000);
