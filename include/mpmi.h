@@ -58,7 +58,9 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
        MPMI_VARIANT_FORCE_BINNING = 8,  /* order them even for small N                        */
        MPMI_VARIANT_LATENCY = 16,       /* several lanes per candidate (d <= 32), any N       */
        MPMI_VARIANT_LAT_R2 = 32,        /* latency kernel: 2 rows per lane                    */
-       MPMI_VARIANT_LAT_R4 = 64 };      /* latency kernel: 4 rows per lane                    */
+       MPMI_VARIANT_LAT_R4 = 64,        /* latency kernel: 4 rows per lane                    */
+       MPMI_VARIANT_NO_TENSOR = 128 };  /* d = 128: FP32 SIMT tile kernel instead of the 3xTF32
+                                           tcgen05 kernel (results agree within the tolerances) */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:
@@ -131,7 +133,8 @@ typedef struct {
 typedef struct {
     int32_t  d_pad;           /* internal padded lifted dim (zero rows / columns: exact)            */
     int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = warp-tile FFMA2 (d<=128),
-                                 3 = latency kernel, 4 lanes per candidate (d<=32, small N)          */
+                                 3 = latency kernel, 4 lanes per candidate (d<=32, small N),
+                                 4 = 3xTF32 tcgen05 tensor-core kernel (d_pad = 128)                 */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;
     int32_t  binning_cells;   /* 0 = candidates walked in index order; else cells of the spatial pre-sort */

@@ -92,6 +92,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 #define MPMI_DECL_TILE(D) KernFn mpmi_pick_tile_##D##_tick(int M, int *smem); KernFn mpmi_pick_tile_##D##_batch(int M, int *smem);
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
+KernFn mpmi_pick_tc_tick(int *smem, int *threads); KernFn mpmi_pick_tc_batch(int *smem, int *threads);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
 KernFn pick_reg(int D, int M, int P, int mode) {
@@ -124,7 +125,7 @@ void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cuda
     long long blocks = (ncand + cpb - 1) / cpb;
     if (blocks < 1) blocks = 1;
     KArgs a = a0;
-    if (c->variant == 2) {                       // persistent warp-tile kernel: one CTA per SM
+    if (c->variant == 2 || c->variant == 4) {    // persistent warp-tile / tensor-core kernel: one CTA per SM
         if (blocks > c->sm_count) blocks = c->sm_count;
         a.st = c->d_state; a.work = &c->d_state->work;
     }
@@ -150,7 +151,7 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
 unsigned grid_for(const mpmi_ctx *c, long long ncand) {
     long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
     if (blocks < 1) blocks = 1;
-    if (c->variant == 2 && blocks > c->sm_count) blocks = c->sm_count;
+    if ((c->variant == 2 || c->variant == 4) && blocks > c->sm_count) blocks = c->sm_count;
     return (unsigned)blocks;
 }
 
@@ -170,7 +171,7 @@ void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **
 int build_graph(mpmi_ctx *c) {
     c->ga = KArgs{};
     c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1;
-    if (c->variant == 2) c->ga.work = &c->d_state->work;
+    if (c->variant == 2 || c->variant == 4) c->ga.work = &c->d_state->work;
     c->tick_grid = grid_for(c, c->dc.shard_count);
     CU(c, cudaGraphCreate(&c->graph, 0));
     cudaKernelNodeParams p; void *args[2];
@@ -417,11 +418,23 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             c->block = 64; c->cand_per_block = 64 / (D / R);     // D/R lanes per candidate
         }
     } else {
-        c->variant = 2;
-        c->P = 1; c->block = kTileThreads; c->cand_per_block = kTileNC;
+        // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)
+        // unless the caller asks for the FP32 SIMT tile kernel; d = 64 stays on the SIMT tile kernel
+        const bool tensor = D == 128 && !(cfg->variant & MPMI_VARIANT_NO_TENSOR);
+        c->P = 1;
+        if (tensor) {
+            c->variant = 4;
+            int threads = 0;
+            c->k_tick = mpmi_pick_tc_tick(&c->smem, &threads);
+            c->k_batch = mpmi_pick_tc_batch(&c->smem, &threads);
+            c->block = threads; c->cand_per_block = 128;
+        } else {
+            c->variant = 2;
+            c->block = kTileThreads; c->cand_per_block = kTileNC;
+            c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem);
+            c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem);
+        }
         c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
-        c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem);
-        c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem);
         if (c->k_tick) {
             CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
             CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
@@ -444,7 +457,7 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->d_pad = c->dc.D; o->variant = c->variant; o->cand_per_block = c->cand_per_block;
     o->threads_per_block = c->block;
     o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
-    if (c->variant == 2 && o->blocks > c->sm_count) o->blocks = c->sm_count;
+    if ((c->variant == 2 || c->variant == 4) && o->blocks > c->sm_count) o->blocks = c->sm_count;
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
     o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = c->binning ? 3 : 1; o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;

@@ -1,0 +1,383 @@
+// rollout_tc.cuh -- tensor-core rollout kernel for padded lifted dim D = 128 (a1-a7, a9), sm_100a.
+//
+// At d = 128 one rollout step of a tile of 128 candidates IS a dense contraction
+// Z'[128 x 128] = [Z | U][128 x 136] * [K | B | 0]^T ("a single matrix-matrix
+// multiplication").  Plain TF32 fails the 1e-4 trajectory tolerance, so every step
+// is computed as the 3xTF32 split product
+//     Z' = Z_hi * K_hi + Z_hi * K_lo + Z_lo * K_hi,      x_hi = x with the low 13 mantissa bits
+// cleared, x_lo = x - x_hi (exact in fp32); the dropped x_lo * k_lo term is 2^-22 relative.
+// tcgen05.mma reads TF32 operands by IGNORING the low 13 bits of the fp32 word (measured), so the
+// fp32 accumulator tile itself serves as the A operand Z_hi of the next step:
+//
+//   TMEM (512 columns x 128 lanes, lane = candidate):  D0 | D1 (ping-pong fp32 state / accumulator)
+//        | A_lo (128 cols) | U_hi (8) | U_lo (8)
+//   shared memory: K_hi and K_lo as K-major no-swizzle B operands ([K | B | 0], 128 x 136 fp32 each).
+//
+// Warp roles: warps 0..7 are "state" warps -- warp e owns TMEM lanes 32*(e%4).. and columns
+// 64*(e/4)..: after every step they read the new state with tcgen05.ld (thread = one candidate,
+// so the safe test is thread-local), write Z_lo back with tcgen05.st and hand the
+// tile back through an mbarrier; warp 8 (one elected lane) issues the MMAs: the two Z_hi products
+// of step s+1 need only the accumulator of step s, so they run WHILE the state warps test and
+// split step s; only Z_lo * K_hi waits for them.  Tiles of 128 candidates are fetched from a
+// global counter (persistent CTAs, one per SM); a tile stops when none of its candidates is alive.
+#pragma once
+#include "mpmi_device.cuh"
+#include "kernel_args.cuh"
+#include "rollout_reg.cuh"
+#include "tcgen05.cuh"
+
+namespace mpmi {
+
+constexpr int kTcD = 128;                         // padded lifted dim
+constexpr int kTcKD = 136;                        // contraction length: 128 state + 8 input columns (m <= 4, zero padded)
+constexpr int kTcTile = 128;                      // candidates per tile = TMEM lanes
+constexpr int kTcStateWarps = 8;
+constexpr int kTcThreads = (kTcStateWarps + 1) * 32;
+constexpr int kTcLBO = 128;                       // bytes between 16-byte K chunks (core matrices contiguous along K)
+constexpr int kTcSBO = (kTcKD / 4) * 128;         // bytes between 8-row groups
+constexpr int kTcImg = (kTcD / 8) * kTcSBO;       // bytes of one B-operand image (69,632)
+constexpr int kTcSmemBytes = 2 * kTcImg;
+constexpr uint32_t kTcColD0 = 0, kTcColD1 = 128, kTcColAlo = 256, kTcColUhi = 384, kTcColUlo = 392;
+
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+// x_lo = x - x_hi (exact) has up to 13 significant bits and the tensor core keeps 11 by TRUNCATION, a bias
+// toward zero of ~2^-22 |x| per operand that adds up coherently over the horizon.  Adding half a TF32 ulp
+// to the bit pattern first turns the hardware's truncation into round-half-away (one integer add).
+__device__ __forceinline__ uint32_t tf32_lo(float x) { return __float_as_uint(x - tf32_hi(x)) + 0x1000u; }
+
+// Same decision as safe_check (rollout_reg.cuh) -- box strict, annulus closed, NaN / Inf unsafe -- but without
+// the 2*nbox-long chain of dependent predicate ANDs (~13 cycles per link), which sits on the per-step critical
+// path here: lo < x < hi  <=>  min(x - lo, hi - x) > 0 (the sign of an fp32 difference is exact); the minimum
+// over all tested dims is a NaN-propagating tree (min.NaN), and NaN fails the final comparison.
+__device__ __forceinline__ float min_nan(float a, float b) {
+    float d;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+    return d;
+}
+template <int NB, int J0, int J1>
+__device__ __forceinline__ float box_slack(const DevCfg &cfg, const float (&x)[NB]) {
+    if constexpr (J1 - J0 == 1) {
+        return min_nan(__fsub_rn(x[J0], cfg.blo[J0]), __fsub_rn(cfg.bhi[J0], x[J0]));
+    } else {
+        constexpr int JM = (J0 + J1) / 2;
+        return min_nan(box_slack<NB, J0, JM>(cfg, x), box_slack<NB, JM, J1>(cfg, x));
+    }
+}
+template <int NB>
+__device__ __forceinline__ bool safe_check_par(const DevCfg &cfg, const float (&x)[NB], int nbox) {
+    static_assert(NB == 16, "tensor-core kernel: 16 physical-state columns");
+    float m = __int_as_float(0x7f800000);
+    if (nbox > 0) {
+        m = box_slack<NB, 0, 2>(cfg, x);
+        if (nbox > 2) {
+            m = min_nan(m, box_slack<NB, 2, 4>(cfg, x));
+            if (nbox > 4) {
+                m = min_nan(m, box_slack<NB, 4, 8>(cfg, x));
+                if (nbox > 8) m = min_nan(m, box_slack<NB, 8, 16>(cfg, x));
+            }
+        }
+    }
+    bool ok = m > 0.f;
+    if (cfg.annulus) {
+        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
+        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
+        ok = ok && (r2 >= cfg.rmin2) && (r2 <= cfg.rmax2);
+    }
+    return ok;
+}
+
+struct TcShared {
+    unsigned long long bar_full, bar_alo, bar_tile;
+    uint32_t tmem_base;
+    unsigned tile[2];
+    unsigned stop_tile;
+    unsigned warp_alive[4];
+    float z0[kTcD];
+};
+
+template <int MODE>
+__global__ void __launch_bounds__(kTcThreads, 1)
+rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
+    using namespace tc;
+    extern __shared__ __align__(1024) unsigned char smem_img[];      // K_hi image | K_lo image
+    __shared__ TcShared sh;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned long long tick = a.tick_val;
+    const float *x0p = a.inline_inputs ? a.x0_val : a.x0;
+    const float *uup = a.inline_inputs ? a.u_val : a.u_user;
+    const int H = (MODE == MODE_TICK) ? cfg.H : a.H;
+    const long long ncand = (MODE == MODE_TICK) ? cfg.shard_count : a.ncand;
+    const bool shared_x0 = (MODE == MODE_TICK) || a.x0_count == 1;
+    const unsigned ntile = (unsigned)((ncand + kTcTile - 1) / kTcTile);
+
+    // ---- one-off: B-operand images [K | B | 0] split into hi / lo, TMEM, barriers, shared lift
+    for (int e = tid; e < kTcD * kTcKD; e += kTcThreads) {
+        const int r = e % kTcD, c = e / kTcD;                        // K[r][c] = KTa[c][r]; rows D.. are B's columns
+        const float v = c < kTcD + cfg.m ? cfg.KTa[c * kTcD + r] : 0.f;
+        const float hi = tf32_hi(v);
+        const int off = (r >> 3) * kTcSBO + (c >> 2) * kTcLBO + (r & 7) * 16 + (c & 3) * 4;
+        *reinterpret_cast<float *>(smem_img + off) = hi;
+        *reinterpret_cast<uint32_t *>(smem_img + kTcImg + off) = tf32_lo(v);
+    }
+    float u_h[kMaxM] = {0.f, 0.f, 0.f, 0.f};
+    bool inputs_ok = true;
+    if (MODE == MODE_TICK) {
+        inputs_ok = finite_inputs(cfg, x0p, uup);
+        clamp_user(cfg, uup, u_h);
+    }
+    if (shared_x0)
+        for (int f = tid; f < kTcD; f += kTcThreads) sh.z0[f] = lift_feature(cfg, f, x0p);
+    if (warp == kTcStateWarps) tmem_alloc<512>(smem_u32(&sh.tmem_base));
+    if (tid == 0) {
+        mbar_init(smem_u32(&sh.bar_full), 1);
+        mbar_init(smem_u32(&sh.bar_alo), kTcStateWarps * 32);
+        mbar_init(smem_u32(&sh.bar_tile), 1);
+        sh.stop_tile = 0xFFFFFFFFu;
+        fence_barrier_init();
+    }
+    fence_proxy_async_smem();
+    fence_before_sync();
+    __syncthreads();
+    fence_after_sync();
+    const uint32_t tb = sh.tmem_base;
+    const uint32_t bar_full = smem_u32(&sh.bar_full), bar_alo = smem_u32(&sh.bar_alo), bar_tile = smem_u32(&sh.bar_tile);
+
+    unsigned long long key = kKeyNone;
+    unsigned n_safe = 0, n_exec = 0;
+
+    if (warp == kTcStateWarps) {
+        // ================= MMA issuer: one elected lane ==============================================
+        if (lane == 0) {
+            const uint32_t idesc = idesc_tf32(kTcTile, kTcD);
+            const uint64_t dhi = smem_desc_kmajor(smem_u32(smem_img), kTcLBO, kTcSBO);
+            const uint64_t dlo = smem_desc_kmajor(smem_u32(smem_img + kTcImg), kTcLBO, kTcSBO);
+            constexpr uint64_t kstep = (2 * kTcLBO) >> 4;                 // descriptor address units per k-block
+            unsigned p_full = 0, p_alo = 0, it = 0;
+#ifdef MPMI_TC_DEBUG
+            long long tw_full = 0, ti_1 = 0, tw_alo = 0, ti_23 = 0, nsteps = 0, tq = 0;
+#define TCT(acc) do { long long t_ = clock64(); acc += t_ - tq; tq = t_; } while (0)
+#else
+#define TCT(acc) do {} while (0)
+#endif
+            for (;; it++) {
+                const unsigned tile = atomicAdd(a.work, 1u);
+                sh.tile[it & 1] = tile;
+                mbar_arrive(bar_tile);
+                if (tile >= ntile) break;
+                for (int s = 0; s < H; s++) {
+                    const uint32_t dcur = tb + ((s & 1) ? kTcColD1 : kTcColD0), dnxt = tb + ((s & 1) ? kTcColD0 : kTcColD1);
+#ifdef MPMI_TC_DEBUG
+                    tq = clock64(); nsteps++;
+#endif
+                    // z_s complete in TMEM: written by the previous step's MMAs (s > 0) or by the prologue (s = 0)
+                    if (s > 0) { mbar_wait(bar_full, p_full); p_full ^= 1; }
+                    else { mbar_wait(bar_alo, p_alo); p_alo ^= 1; }
+                    fence_after_sync();
+                    TCT(tw_full);
+                    // The small products go first: the tensor core accumulates with truncation toward zero
+                    // (measured), so terms added while the accumulator is still ~2^-11 |z| lose nothing that
+                    // matters, and only the 17 accumulations of Z_hi * K_hi run at full magnitude.
+                    if (s == 0 && !(sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3])) {
+                        sh.stop_tile = tile; mbar_arrive(bar_full); break;                  // nothing valid in this tile
+                    }
+                    constexpr int kSplit = 12;                             // k-blocks of group 1 issued before the hand-back wait
+#pragma unroll
+                    for (int kk = 0; kk < kSplit; kk++)                    // Z_hi * K_lo  (Z_hi = the fp32 state itself)
+                        mma_tf32_ts(dnxt, dcur + 8 * kk, dlo + kk * kstep, idesc, kk > 0);
+                    TCT(ti_1);
+                    if (s > 0) {                                           // state warps: z_s tested, Z_lo written
+                        mbar_wait(bar_alo, p_alo); p_alo ^= 1;             // (its latency hides behind the queued MMAs)
+                        fence_after_sync();
+                        if (!(sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3])) {
+                            sh.stop_tile = tile; mma_commit(bar_full); break;               // stop: drains, then wakes them
+                        }
+                    }
+                    TCT(tw_alo);
+#pragma unroll
+                    for (int kk = kSplit; kk < 17; kk++)
+                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColUhi, dlo + kk * kstep, idesc, true);
+#pragma unroll
+                    for (int kk = 0; kk < 17; kk++)                        // Z_lo * K_hi
+                        mma_tf32_ts(dnxt, kk < 16 ? tb + kTcColAlo + 8 * kk : tb + kTcColUlo, dhi + kk * kstep, idesc, true);
+#pragma unroll
+                    for (int kk = 0; kk < 17; kk++)                        // Z_hi * K_hi
+                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColUhi, dhi + kk * kstep, idesc, true);
+                    mma_commit(bar_full);
+                    TCT(ti_23);
+                }
+                mbar_wait(bar_full, p_full); p_full ^= 1;                 // last commit (or the stop signal) of this tile
+            }
+#ifdef MPMI_TC_DEBUG
+            if (blockIdx.x == 0 && nsteps > 0)
+                printf("tc timing (clk/step): wait_full %lld issue1 %lld wait_alo %lld issue23 %lld  steps %lld\n",
+                       tw_full / nsteps, ti_1 / nsteps, tw_alo / nsteps, ti_23 / nsteps, nsteps);
+#endif
+        }
+        __syncwarp();
+    } else {
+        // ================= state warps: thread = (candidate row, column half) ===========================
+        const int q = warp & 3, hc = warp >> 2;                          // TMEM lane quadrant, column half
+        const int row = q * 32 + lane;
+        const uint32_t tlane = tb + ((uint32_t)(q * 32) << 16);
+        const int c0 = hc * 64;
+        constexpr int NB = kMaxN;
+        const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
+        const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
+        const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
+        const float qnan = __int_as_float(0x7fc00000);
+        unsigned p_full = 0, p_tile = 0;
+        for (unsigned it = 0;; it++) {
+            mbar_wait(bar_tile, p_tile); p_tile ^= 1;
+            const unsigned tile = sh.tile[it & 1];
+            if (tile >= ntile) break;
+
+            // ---- a1 + a2: this thread's candidate, its half of z_0 and (column half 0) its input
+            long long li = (long long)tile * kTcTile + row;
+            if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];       // spatially ordered walk
+            const bool valid = li < ncand && inputs_ok;
+            bool alive = valid;
+            int steps = 0;
+            float u[kMaxM] = {0.f, 0.f, 0.f, 0.f};
+            if (li < ncand) {
+                if (MODE == MODE_BATCH && a.U) {
+                    for (int j = 0; j < cfg.m; j++) u[j] = a.U[li * cfg.m + j];
+                } else {
+                    sample_u(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, tick, u_h, u);
+                }
+            }
+            __syncwarp();                                                // tcgen05.st / ld below are .sync.aligned
+            {
+                float x[kMaxN];
+                if (!shared_x0) {
+                    const long long r0 = li < ncand ? li : 0;
+                    for (int j = 0; j < kMaxN; j++) x[j] = j < cfg.n ? a.x0[r0 * cfg.n + j] : 0.f;
+                }
+#pragma unroll 1
+                for (int cc = 0; cc < 64; cc += 16) {
+                    uint32_t v[16], lo[16];
+#pragma unroll
+                    for (int j = 0; j < 16; j++) {
+                        const float z = shared_x0 ? sh.z0[c0 + cc + j] : lift_feature(cfg, c0 + cc + j, x);
+                        v[j] = __float_as_uint(z);
+                        lo[j] = tf32_lo(z);
+                    }
+                    tmem_st16(tlane + kTcColD0 + c0 + cc, v);
+                    tmem_st16(tlane + kTcColAlo + c0 + cc, lo);
+                }
+                if (hc == 0) {
+                    uint32_t uh[8], ul[8];
+#pragma unroll
+                    for (int j = 0; j < 8; j++) {
+                        const float uj = j < kMaxM ? u[j < kMaxM ? j : 0] : 0.f;
+                        uh[j] = __float_as_uint(uj);
+                        ul[j] = tf32_lo(uj);
+                    }
+                    tmem_st8(tlane + kTcColUhi, uh);
+                    tmem_st8(tlane + kTcColUlo, ul);
+                    const bool any = __any_sync(0xffffffffu, alive);
+                    if (lane == 0) sh.warp_alive[q] = any ? 1u : 0u;
+                }
+            }
+            wait_st();
+            fence_before_sync();
+            mbar_arrive(bar_alo);
+
+            // ---- a3 + a4: after MMA step s-1 the accumulator holds z_s; test it, split it, hand it back
+            int s = 1;
+            for (; s <= H; s++) {
+                mbar_wait(bar_full, p_full); p_full ^= 1;
+                fence_after_sync();
+                if (*reinterpret_cast<volatile unsigned *>(&sh.stop_tile) == tile) break;
+                const uint32_t dcol = (s & 1) ? kTcColD1 : kTcColD0;
+                const bool was_alive = alive;
+                __syncwarp();
+                // this thread's 64 columns of z_s: four loads in flight, one wait
+                uint32_t r[64];
+#pragma unroll
+                for (int cc = 0; cc < 64; cc += 16) tmem_ld16(tlane + dcol + c0 + cc, *reinterpret_cast<uint32_t(*)[16]>(&r[cc]));
+                uint32_t rp[16];                                         // the physical state sits in columns 0..15
+                if (dump && hc != 0) tmem_ld16(tlane + dcol, rp);
+                wait_ld();
+                if (hc == 0 || dump) {
+                    float x[NB];
+#pragma unroll
+                    for (int j = 0; j < NB; j++) x[j] = __uint_as_float(hc == 0 ? r[j] : rp[j]);
+                    alive = safe_check_par<NB>(cfg, x, nbox) && was_alive;
+                    steps += alive ? 1 : 0;
+                }
+                if (hc == 0) {
+                    const bool any = __any_sync(0xffffffffu, alive);
+                    if (lane == 0) sh.warp_alive[q] = any ? 1u : 0u;
+                }
+                if (s < H) {
+#pragma unroll
+                    for (int cc = 0; cc < 64; cc += 8) {
+                        uint32_t lo[8];
+#pragma unroll
+                        for (int j = 0; j < 8; j++) lo[j] = tf32_lo(__uint_as_float(r[cc + j]));
+                        tmem_st8(tlane + kTcColAlo + c0 + cc, lo);
+                    }
+                }
+                if (dump && li < ncand) {                                // a9: traj[(k*J + row)*Ncand + i], k = s-1
+#pragma unroll
+                    for (int j = 0; j < 64; j++) {
+                        const int ji = c0 + j;
+                        const int orow = ji < cfg.n ? (int)cfg.perm[ji < kMaxN ? ji : 0] : ji;
+                        if (orow < J)
+                            a.traj[((long long)(s - 1) * J + orow) * ncand + li] = was_alive ? __uint_as_float(r[j]) : qnan;
+                    }
+                }
+                if (s < H) {
+                    wait_st();
+                    fence_before_sync();
+                    mbar_arrive(bar_alo);
+                }
+            }
+            if (dump && li < ncand) {                                    // states after the tile stopped: NaN
+                for (int k = s - 1; k < H; k++)
+                    for (int j = 0; j < 64; j++) {
+                        const int ji = c0 + j;
+                        const int orow = ji < cfg.n ? (int)cfg.perm[ji < kMaxN ? ji : 0] : ji;
+                        if (orow < J) a.traj[((long long)k * J + orow) * ncand + li] = qnan;
+                    }
+            }
+            if (hc == 0) {
+                if (MODE == MODE_BATCH) {
+                    if (li < ncand) {
+                        a.steps[li] = steps;
+                        if (a.safe) a.safe[li] = steps == H ? 1 : 0;
+                    }
+                } else if (valid) {                                      // a5: this candidate's key
+                    const bool safe = steps == H;
+                    float d2 = 0.f;
+#pragma unroll
+                    for (int j = 0; j < kMaxM; j++) {
+                        const float df = __fsub_rn(u[j], u_h[j]);
+                        d2 = __fmaf_rn(df, df, d2);
+                    }
+                    const unsigned long long kk = make_key(safe, d2, H, steps, cfg.shard_begin + li);
+                    key = kk < key ? kk : key;
+                    n_safe += safe ? 1u : 0u;
+                    n_exec += (unsigned)(steps + 1 < H ? steps + 1 : H);
+                }
+            }
+        }
+    }
+
+    // ---- teardown: all MMAs of this CTA have completed (the state warps waited for the last commit)
+    fence_before_sync();
+    __syncthreads();
+    if (warp == kTcStateWarps) tc::tmem_dealloc<512>(tb);
+    if (MODE == MODE_BATCH) {
+        if (tid == 0) {                          // the last CTA to finish re-arms the work counter for the next launch
+            __threadfence();
+            if (atomicAdd(&a.st->ticket, 1u) == gridDim.x - 1) { *a.work = 0u; a.st->ticket = 0u; __threadfence(); }
+        }
+        return;
+    }
+    // ---- a6 + a7
+    block_select_and_finalise<kTcStateWarps + 1>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, a.work);
+}
+
+}  // namespace mpmi

@@ -50,7 +50,9 @@ def test_sampler_bit_exact(mp, name):
     w.u_lo = np.array([-1.0, 0.0, -1.0][: w.m], np.float32); w.u_hi = np.array([1.0, 1.0, 0.0][: w.m], np.float32)
     w.seed = 0xDEADBEEF12345
     o = _oracle(w)
-    ctx = mp.Context(w)
+    # d = 128: the FP32 SIMT kernel exposes the candidates exactly; the 3xTF32 tensor-core kernel draws
+    # the same candidates but its step keeps 22 mantissa bits of u (hi + truncated lo), checked below
+    ctx = mp.Context(w, variant=mp.mpmi.VARIANT_NO_TENSOR)
     N = w.N
     X0 = _dev(w.x_nom[None, :])
     traj = torch.empty((1, w.d, N), dtype=torch.float32, device="cuda")
@@ -61,6 +63,14 @@ def test_sampler_bit_exact(mp, name):
         got = traj[0, : w.m, :].T.cpu().numpy()
         ref = o.sample(tick, np.arange(N))
         assert np.array_equal(got.view(np.uint32), ref.view(np.uint32))
+    if name == "C5":
+        tc = mp.Context(w)
+        assert tc.info()["variant"] == 4
+        tc.rollout_batch(0, X0.data_ptr(), 1, N, 1, mp.DUMP_LIFTED, traj.data_ptr(), steps.data_ptr(), 0, tick=0)
+        torch.cuda.synchronize()
+        got = traj[0, : w.m, :].T.cpu().numpy().astype(np.float64)
+        ref = o.sample(0, np.arange(N)).astype(np.float64)
+        assert np.max(np.abs(got - ref) / np.maximum(np.abs(ref), 1e-30)) <= 2.0 ** -21
 
 
 # ------------------------------------------------------------------ a2: lift ------------------------
