@@ -178,6 +178,7 @@ def main():
     ap.add_argument("--no-latency", action="store_true")
     ap.add_argument("--dump", choices=["lifted", "phys"], default=None,
                     help="measure the trajectory-dump path (mpmi_rollout_batch, SURVEY 8(a) a9) instead of the tick")
+    ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
     ap.add_argument("--bounds-scale", type=float, default=1.0,
                     help="scale the safe set (100 = every rollout safe: no early exit, full N*H work)")
     args = ap.parse_args()
@@ -211,7 +212,8 @@ def main():
     x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
     begin, count = shard_plan(w.N, 1, world, rank)             # the injected u_user (index N) goes to the last rank
-    ctx = mp.Context(w, device=local, shard=(begin, count) if world > 1 else (0, 0))
+    ctx = mp.Context(w, device=local, shard=(begin, count) if world > 1 else (0, 0),
+                     variant=mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0)
     info = ctx.info()
     stream = torch.cuda.current_stream().cuda_stream
     if args.dump:
@@ -313,11 +315,27 @@ def main():
             f = line.split(",")
             if f and f[0] == args.workload:
                 traffic = int(f[2])
-    roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
-                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
-                "kernel": "rollout_reg_kernel" if info["variant"] == 1 else "rollout_tile_kernel",
-                "nominal_frac": nominal / K_ / max(world, 1) * flop / (total_ms * 1e-3 / K_) / 1e12 / FP32_PEAK_TFLOPS}
+    nominal_frac = nominal / K_ / max(world, 1) * flop / (total_ms * 1e-3 / K_) / 1e12 / FP32_PEAK_TFLOPS
+    if info["variant"] == 4:
+        # d = 128 runs as a 3xTF32 split contraction on the tcgen05 tensor cores (rollout_tc.cuh): every
+        # algorithmic flop costs three TF32 tensor flops, so the peak for this path is the measured bf16
+        # GEMM peak x the guide's nominal tf32:bf16 ratio (1.1 : 2.25 PFLOP/s) / 3.
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+        bf16 = float(peaks.get("bf16_tflops", 1590.0))
+        peak = bf16 * (1.1 / 2.25) / 3.0
+        roofline = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "traffic": traffic,
+                    "peak_source": ("MEASURED_PEAKS.json bf16_tflops (burst; of measured)" if peaks else "fallback 1590 TFLOP/s bf16 (of fallback)")
+                                   + " x 1.1/2.25 (nominal tf32:bf16) / 3 (3xTF32 split products per algorithmic flop)",
+                    "kernel": "rollout_tc_kernel", "dtype": "3xTF32 (fp32 accumulate)",
+                    "tensor_tflops_executed": achieved * 3.0 * 136.0 / (w.d + w.m),
+                    "fp32_alu_frac": achieved / FP32_PEAK_TFLOPS, "nominal_fp32_alu_frac": nominal_frac}
+    else:
+        roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+                    "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
+                    "kernel": "rollout_reg_kernel" if info["variant"] == 1 else "rollout_tile_kernel",
+                    "nominal_frac": nominal_frac}
 
     if rank != 0:
         if dist:
@@ -341,7 +359,7 @@ def main():
     out = {
         "metric": "rollout sample-steps/s", "value": value, "unit": "sample-steps/s", "n_gpus": world,
         "steps": K_, "warmup": W_, "ms_per_step": total_ms / K_, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f32 (3xTF32 split products, fp32 accumulate)" if info["variant"] == 4 else "f32", "data": "synthetic",
         "config": {"workload": f"{args.workload}: n={w.n} m={w.m} d={w.d} N={n_per}/GPU (+1 user slot) H={w.H}, "
                                f"Philox/grid sampler, calibrated 40% safe (DESIGN.md section 4)"
                                + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else ""),
