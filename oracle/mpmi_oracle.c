@@ -129,17 +129,47 @@ int orc_is_safe(const orc_config *c, const double *x, double *margin) {
     return safe;
 }
 
+/* ---- the additive noise z_i of Algorithm 2 l.5, "x_p <- f(x_p, xi(i)) + z_i" with z_i i.i.d.
+ *      Gaussian white noise.  The paper fixes neither the generator nor the
+ *      variance; DESIGN G17: eps ~ N(0, I_n) on the n physical dims, one independent draw per
+ *      (tick, candidate i, step k, dim), from the counter-based Philox4x32-10 stream
+ *      key = (seed_lo, seed_hi ^ 0x6E6F6973), counter = (i, (q << 16) | k, tick_lo, tick_hi), q = dim / 4,
+ *      turned into normals by the Box-Muller transform: words (w0, w1) -> dims 4q, 4q+1 and
+ *      (w2, w3) -> dims 4q+2, 4q+3, with u1 = ((w >> 8) + 1) 2^-24 in (0, 1], u2 = (w' >> 8) 2^-24. */
+void orc_noise(const orc_config *c, uint64_t tick, int64_t i, int k, double *eps) {
+    const double two_pi = 6.283185307179586476925286766559;
+    const uint32_t key[2] = { (uint32_t)c->seed, (uint32_t)(c->seed >> 32) ^ 0x6E6F6973u };
+    for (int q = 0; 4 * q < c->n; q++) {
+        const uint32_t ctr[4] = { (uint32_t)i, ((uint32_t)q << 16) | (uint32_t)k, (uint32_t)tick, (uint32_t)(tick >> 32) };
+        uint32_t w[4];
+        orc_philox4x32_10(ctr, key, w);
+        for (int h = 0; h < 2; h++) {
+            const double u1 = ((double)(w[2 * h] >> 8) + 1.0) * 0x1p-24;
+            const double u2 = (double)(w[2 * h + 1] >> 8) * 0x1p-24;
+            const double r = sqrt(-2.0 * log(u1));
+            const int j = 4 * q + 2 * h;
+            if (j < c->n)     eps[j]     = r * cos(two_pi * u2);
+            if (j + 1 < c->n) eps[j + 1] = r * sin(two_pi * u2);
+        }
+    }
+}
+
 /* ---- Algorithm 2 lines 3-8 for ONE candidate.
  *      x_t itself is not tested; exactly H predicted states x_1..x_H (DESIGN G8).
- *      f(x_p, xi) is the linear lifted model z' = K z + B u, x = z[0:n] (DESIGN G5); the
- *      same input is held over the horizon; noise z_i = 0 (DESIGN G6).
+ *      f(x_p, xi): ORC_MODEL_LINEAR  z' = K z + B u, x = z[0:n], lifted once (DESIGN G5);
+ *                  ORC_MODEL_RELIFT  x' = C (K Psi(x) + B u): the physical state is re-lifted
+ *                  before every step, the literal f(x, u) on states of PAPER.md:132 (DESIGN G18).
+ *      The same input is held over the horizon.  If noise_sigma > 0 the noise
+ *      sigma * eps_k is added to the n physical rows of the predicted state BEFORE isSafe, as in
+ *      l.5-6 of the algorithm, and stays in the state that is carried on.
  *      Returns steps = number of safe predicted states before the first violation (H <=> safe).
  *      margin = min |g| over every state tested, including the violating one.
  *      traj (optional): z_1..z_e written at traj[k*d + f], e = min(steps+1, H); the rest NaN. */
-int orc_rollout(const orc_config *c, const double *z0, const double *u, int H,
+int orc_rollout(const orc_config *c, const double *z0, const double *u, int H, uint64_t tick, int64_t i,
                 double *margin, double *traj) {
-    const int d = c->d, m = c->m;
+    const int d = c->d, m = c->m, n = c->n;
     double *z = (double *)malloc(sizeof(double) * d), *zn = (double *)malloc(sizeof(double) * d);
+    double eps[64];
     memcpy(z, z0, sizeof(double) * d);
     double mg = INFINITY;
     int steps = H, safe = 1, k = 0;
@@ -151,7 +181,12 @@ int orc_rollout(const orc_config *c, const double *z0, const double *u, int H,
             for (int j = 0; j < m; j++) s += c->B[r * m + j] * u[j];
             zn[r] = s;
         }
-        memcpy(z, zn, sizeof(double) * d);
+        if (c->noise_sigma > 0.0) {                           /* l.5: ... + z_i                */
+            orc_noise(c, tick, i, k, eps);
+            for (int j = 0; j < n; j++) zn[j] += c->noise_sigma * eps[j];
+        }
+        if (c->model_kind == ORC_MODEL_RELIFT) orc_lift(c, zn, z);   /* carry x = C zn, re-lifted */
+        else memcpy(z, zn, sizeof(double) * d);
         if (traj) memcpy(traj + (long)k * d, z, sizeof(double) * d);
         double g;
         safe = orc_is_safe(c, z, &g);                         /* l.6: safe = isSafe(x_p)       */
@@ -195,7 +230,7 @@ int orc_step(const orc_config *c, const float *x0, const float *u_user, uint64_t
             s2 += df * df;
         }
         dist[i] = sqrt(s2);                                    /* cost = Euclidean distance */
-        steps[i] = orc_rollout(c, z0, ud, H, &marg[i], NULL);  /* l.3-8 */
+        steps[i] = orc_rollout(c, z0, ud, H, tick, i, &marg[i], NULL);  /* l.3-8 */
     }
 
     /* l.9-13: store <- safe xi(i);  u_r <- argmin cost over store; ties -> lower index.
@@ -224,7 +259,7 @@ int orc_step(const orc_config *c, const float *x0, const float *u_user, uint64_t
 
 /* ---- rollouts for caller-supplied inputs (trajectory cloud of Fig. 1) ---- */
 int orc_rollout_batch(const orc_config *c, const float *U, const float *X0, int x0_count,
-                      int64_t Ncand, int H, int32_t *steps, double *margin, double *traj) {
+                      int64_t Ncand, int H, uint64_t tick, int32_t *steps, double *margin, double *traj) {
     const int d = c->d, m = c->m, n = c->n;
     if (x0_count != 1 && x0_count != Ncand) return -1;
     #pragma omp parallel for schedule(static)
@@ -235,7 +270,7 @@ int orc_rollout_batch(const orc_config *c, const float *U, const float *X0, int 
         for (int j = 0; j < m; j++) ud[j] = (double)U[i * m + j];
         orc_lift(c, xd, z0);
         double mg;
-        steps[i] = orc_rollout(c, z0, ud, H, &mg, traj ? traj + i * (int64_t)H * d : NULL);
+        steps[i] = orc_rollout(c, z0, ud, H, tick, i, &mg, traj ? traj + i * (int64_t)H * d : NULL);
         if (margin) margin[i] = mg;
         free(z0);
     }

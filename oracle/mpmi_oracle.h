@@ -10,7 +10,11 @@
  *
  * Pins (tests/test_oracle_pins.py): closed form z_H = K^H z0 + sum K^k B u, geometric series,
  * brute force on tiny inputs, Philox known-answer vectors, Eq. (2) printed value 0.0001,
- * K=0 / K=rho*I / B=0 special cases, prefix / monotone / shard invariants, lift hand values.
+ * K=0 / K=rho*I / B=0 special cases, prefix / monotone / shard invariants, lift hand values;
+ * noise (NEXT-2): normal moments + Kolmogorov-Smirnov against the normal CDF, closed form
+ * z_H = K^H z0 + sum K^(H-1-k) (B u + E eps_k); re-lift model (NEXT-3): reduction to the textbook
+ * linear recursion x' = A x + B u when K[0:n, n:] = 0, an independent Python loop on a tiny system,
+ * identity lift == linear model.
  * Functions with no pin: none ("parity unpinned" would be stated here).
  */
 #ifndef MPMI_ORACLE_H
@@ -19,6 +23,8 @@
 
 enum { ORC_SAMPLER_PHILOX = 0, ORC_SAMPLER_GRID = 1 };
 enum { ORC_LIFT_MONO = 0, ORC_LIFT_RFF = 1 };
+enum { ORC_MODEL_LINEAR = 0,  /* z' = K z + B u, lifted once, x = z[0:n]                   */
+       ORC_MODEL_RELIFT = 1 };/* x' = C (K Psi(x) + B u): re-lift the physical state every step */
 
 typedef struct {
     int32_t n, m, d, N, H;
@@ -39,6 +45,9 @@ typedef struct {
     int32_t annulus;          /* 1: rmin <= hypot(x[ix]-cx, x[iy]-cy) <= rmax (closed)*/
     int32_t ix, iy; double cx, cy, rmin, rmax;
     double inflate;           /* inflated barrier                      */
+    double noise_sigma;       /* std of the additive Gaussian white noise z_i of Alg. 2 l.5
+                                 (PAPER.md:132, 150), on the physical rows; 0 = none (DESIGN G6, G17) */
+    int32_t model_kind;       /* ORC_MODEL_*: how f(x, u) of PAPER.md:132 is evaluated (DESIGN G5, G18) */
 } orc_config;
 
 typedef struct {
@@ -56,13 +65,14 @@ void   orc_sample(const orc_config *c, uint64_t tick, int64_t i, float *u /* m *
 void   orc_clamp_user(const orc_config *c, const float *u_user, float *u_h);
 void   orc_lift(const orc_config *c, const double *x /* n */, double *z /* d */);
 int    orc_is_safe(const orc_config *c, const double *x /* n */, double *margin);
-int    orc_rollout(const orc_config *c, const double *z0, const double *u, int H,
+void   orc_noise(const orc_config *c, uint64_t tick, int64_t i, int k, double *eps /* n standard normals */);
+int    orc_rollout(const orc_config *c, const double *z0, const double *u, int H, uint64_t tick, int64_t i,
                    double *margin, double *traj /* H*d or NULL */);
 int    orc_step(const orc_config *c, const float *x0, const float *u_user, uint64_t tick,
                 orc_result *res, int32_t *steps /* N+1 or NULL */, double *margin /* N+1 or NULL */,
                 double *dist /* N+1 or NULL */, float *U /* (N+1)*m or NULL */);
 int    orc_rollout_batch(const orc_config *c, const float *U /* Ncand*m */, const float *X0 /* x0_count*n */,
-                         int x0_count, int64_t Ncand, int H, int32_t *steps, double *margin,
+                         int x0_count, int64_t Ncand, int H, uint64_t tick, int32_t *steps, double *margin,
                          double *traj /* Ncand*H*d or NULL */);
 int    orc_num_threads(void);
 #endif

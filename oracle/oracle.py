@@ -35,7 +35,7 @@ class _Cfg(C.Structure):
                 ("nbounds", C.c_int32), ("bidx", C.c_void_p), ("blo", C.c_void_p), ("bhi", C.c_void_p),
                 ("annulus", C.c_int32), ("ix", C.c_int32), ("iy", C.c_int32),
                 ("cx", C.c_double), ("cy", C.c_double), ("rmin", C.c_double), ("rmax", C.c_double),
-                ("inflate", C.c_double)]
+                ("inflate", C.c_double), ("noise_sigma", C.c_double), ("model_kind", C.c_int32)]
 
 
 class _Res(C.Structure):
@@ -96,6 +96,8 @@ class Oracle:
         self.cx, self.cy = f32(g("cx", 0.0)), f32(g("cy", 0.0))
         self.rmin, self.rmax = f32(g("rmin", 0.0)), f32(g("rmax", 0.0))
         self.inflate = f32(g("inflate", 0.0))
+        self.noise_sigma = f32(g("noise_sigma", 0.0))
+        self.model_kind = int(g("model_kind", 0))
         self._cfg = self._make_cfg()
 
     def _make_cfg(self):
@@ -108,6 +110,7 @@ class Oracle:
         c.nbounds, c.bidx, c.blo, c.bhi = len(self.bidx), _p(self.bidx), _p(self.blo), _p(self.bhi)
         c.annulus, c.ix, c.iy = self.annulus, self.ix, self.iy
         c.cx, c.cy, c.rmin, c.rmax, c.inflate = self.cx, self.cy, self.rmin, self.rmax, self.inflate
+        c.noise_sigma, c.model_kind = self.noise_sigma, self.model_kind
         return c
 
     @property
@@ -136,12 +139,19 @@ class Oracle:
         s = lib().orc_is_safe(C.byref(self._cfg), _p(x), C.byref(mg))
         return bool(s), mg.value
 
-    def rollout(self, z0, u, H=None, want_traj=False):
+    def noise(self, tick, i, k):
+        """The n standard normals added (times noise_sigma) to the physical rows of candidate i at step k."""
+        eps = np.empty(self.n, dtype=np.float64)
+        lib().orc_noise(C.byref(self._cfg), C.c_uint64(tick), C.c_int64(int(i)), C.c_int(int(k)), _p(eps))
+        return eps
+
+    def rollout(self, z0, u, H=None, want_traj=False, tick=0, i=0):
         H = self.H if H is None else H
         z0 = np.ascontiguousarray(z0, dtype=np.float64); u = np.ascontiguousarray(u, dtype=np.float64)
         traj = np.empty((H, self.d), dtype=np.float64) if want_traj else None
         mg = C.c_double()
-        steps = lib().orc_rollout(C.byref(self._cfg), _p(z0), _p(u), C.c_int(H), C.byref(mg), _p(traj))
+        steps = lib().orc_rollout(C.byref(self._cfg), _p(z0), _p(u), C.c_int(H), C.c_uint64(tick), C.c_int64(int(i)),
+                                  C.byref(mg), _p(traj))
         return steps, mg.value, traj
 
     def step(self, x0, u_user, tick, detail=False):
@@ -163,7 +173,7 @@ class Oracle:
             out.update(steps_all=steps, margin_all=marg, dist_all=dist, U=U)
         return out
 
-    def rollout_batch(self, U, X0, H=None, want_traj=False):
+    def rollout_batch(self, U, X0, H=None, want_traj=False, tick=0):
         H = self.H if H is None else H
         U = np.ascontiguousarray(U, dtype=np.float32).reshape(-1, self.m)
         X0 = np.ascontiguousarray(X0, dtype=np.float32).reshape(-1, self.n)
@@ -171,7 +181,7 @@ class Oracle:
         steps = np.empty(Nc, dtype=np.int32); marg = np.empty(Nc, dtype=np.float64)
         traj = np.empty((Nc, H, self.d), dtype=np.float64) if want_traj else None
         rc = lib().orc_rollout_batch(C.byref(self._cfg), _p(U), _p(X0), C.c_int(X0.shape[0]), C.c_int64(Nc),
-                                     C.c_int(H), _p(steps), _p(marg), _p(traj))
+                                     C.c_int(H), C.c_uint64(tick), _p(steps), _p(marg), _p(traj))
         if rc != 0:
             raise ValueError("oracle: x0_count must be 1 or N")
         return steps, marg, traj

@@ -359,3 +359,135 @@ def test_calibrated_workloads_are_mixed():
         w = W.make(name, N=2048 if name != "C3" else 10000)
         r = Oracle(w, include_user=0).step(w.x_nom, np.zeros(w.m, np.float32), 0)
         assert 0.28 <= r["n_safe"] / w.N <= 0.50, (name, r["n_safe"] / w.N)
+
+
+# ---------------------------------------------------------------- NEXT-2: prediction noise ---------
+def test_noise_is_standard_normal_and_independent():
+    """eps of orc_noise: N(0, 1) marginals (moments + Kolmogorov-Smirnov against the normal CDF),
+    uncorrelated across dims, steps, candidates and ticks (i.i.d. Gaussian white noise)."""
+    from scipy import stats
+    w = _free(W.make("C4", calibrated=False)); w.noise_sigma = 1.0
+    o = Oracle(w)
+    E = np.array([[o.noise(3, i, k) for k in range(40)] for i in range(700)])          # (cand, step, dim)
+    v = E.reshape(-1)
+    assert abs(v.mean()) < 0.01 and abs(v.var() - 1.0) < 0.02
+    assert abs(stats.kurtosis(v, fisher=False) - 3.0) < 0.06 and abs(stats.skew(v)) < 0.03
+    assert stats.kstest(v, "norm").pvalue > 1e-3
+    for j in range(w.n):                                                              # every dim on its own
+        assert stats.kstest(E[:, :, j].reshape(-1), "norm").pvalue > 1e-4
+    flat = E.reshape(-1, w.n)
+    c = np.corrcoef(flat.T)
+    assert np.abs(c - np.eye(w.n)).max() < 0.02                                       # across dims (incl. Box-Muller pairs)
+    assert abs(np.corrcoef(E[:, :-1, :].reshape(-1), E[:, 1:, :].reshape(-1))[0, 1]) < 0.02   # across steps
+    assert abs(np.corrcoef(E[:-1].reshape(-1), E[1:].reshape(-1))[0, 1]) < 0.02               # across candidates
+    other = np.array([[o.noise(4, i, k) for k in range(40)] for i in range(100)])
+    assert abs(np.corrcoef(other.reshape(-1), E[:100].reshape(-1))[0, 1]) < 0.05               # across ticks
+    uni = np.array([o.sample(3, [i])[0] for i in range(700)])                          # not the sampling stream
+    assert abs(np.corrcoef(uni[:, 0], E[:, 0, 0])[0, 1]) < 0.1
+
+
+@pytest.mark.parametrize("name", ["C1", "C4"])
+def test_noise_rollout_closed_form(name):
+    """z_H = K^H z0 + sum_k K^(H-1-k) (B u + sigma E eps_k), E = [I_n; 0]: pins WHERE the noise enters
+    (physical rows, after the step, kept in the carried state) and which draw belongs to which step."""
+    w = _free(W.make(name, N=8)); w.noise_sigma = 0.05
+    o = Oracle(w)
+    K, B = o.K, o.B
+    z0 = o.lift(w.x_nom.astype(np.float64))
+    H, tick = 12, 9
+    for i in (0, 5):
+        u = o.sample(tick, [i])[0].astype(np.float64)
+        steps, _, traj = o.rollout(z0, u, H=H, want_traj=True, tick=tick, i=i)
+        assert steps == H
+        z = z0.copy()
+        for k in range(H):
+            e = np.zeros(w.d); e[: w.n] = np.float64(np.float32(w.noise_sigma)) * o.noise(tick, i, k)
+            z = K @ z + B @ u + e
+            assert np.allclose(traj[k], z, rtol=1e-12, atol=1e-12)
+        acc = np.linalg.matrix_power(K, H) @ z0
+        for k in range(H):
+            e = np.zeros(w.d); e[: w.n] = np.float64(np.float32(w.noise_sigma)) * o.noise(tick, i, k)
+            acc += np.linalg.matrix_power(K, H - 1 - k) @ (B @ u + e)
+        assert np.allclose(traj[H - 1], acc, rtol=1e-9, atol=1e-9)
+
+
+def test_noise_zero_sigma_and_tick_semantics():
+    """sigma = 0 is the noise-free path bit for bit; the noise is tested BEFORE it can be ignored:
+    K = 0, B = 0 makes x_1 = sigma eps_0, so candidate i is unsafe iff |sigma eps_0| leaves the box."""
+    w = W.make("C1", N=64)
+    a = Oracle(w).step(w.x_nom, np.zeros(1, np.float32), 5, detail=True)
+    w2 = W.make("C1", N=64); w2.noise_sigma = 0.0
+    b = Oracle(w2).step(w2.x_nom, np.zeros(1, np.float32), 5, detail=True)
+    assert np.array_equal(a["steps_all"], b["steps_all"]) and a["index"] == b["index"]
+    w3 = W.make("C1", N=400); w3.K = np.zeros_like(w3.K); w3.B = np.zeros_like(w3.B); w3.noise_sigma = 0.4; w3.H = 1
+    o = Oracle(w3)
+    r = o.step(np.zeros(4, np.float32), np.zeros(1, np.float32), 2, detail=True)
+    sig = float(np.float32(0.4))
+    for i in range(401):
+        x1 = sig * o.noise(2, i, 0)
+        inside = all(lo < x1[j] < hi for j, lo, hi in zip(w3.bidx, w3.blo, w3.bhi))
+        assert (r["steps_all"][i] == 1) == inside
+    assert 0.2 < (r["steps_all"] == 1).mean() < 0.95
+
+
+# ---------------------------------------------------------------- NEXT-3: re-lift model -------------
+def _py_lift_mono(terms, x):
+    out = []
+    for f in range(terms.shape[0]):
+        p = 1.0
+        for code in terms[f]:
+            if code == 0xFF:
+                continue
+            v = x[code & 0x3F]
+            p *= v if code >> 6 == 0 else (np.sin(v) if code >> 6 == 1 else np.cos(v))
+        out.append(p)
+    return np.array(out)
+
+
+def test_relift_matches_independent_python_loop():
+    """x_{k+1} = C (K Psi(x_k) + B u) (the literal f(x, u) on states): an un-vectorised
+    Python restatement on the race-car lift (sin, cos and product features)."""
+    w = _free(W.make("C3", N=16)); w.model_kind = 1
+    o = Oracle(w)
+    x0 = (w.x_nom + 0.01).astype(np.float64)
+    u = np.array([0.3, -0.2])
+    H = 9
+    steps, _, traj = o.rollout(o.lift(x0), u, H=H, want_traj=True)
+    assert steps == H
+    x = x0.copy()
+    for k in range(H):
+        z = _py_lift_mono(w.terms, x)
+        zn = o.K @ z + o.B @ u
+        x = zn[: w.n]
+        assert np.allclose(traj[k][: w.n], x, rtol=1e-11, atol=1e-11)
+        assert np.allclose(traj[k], _py_lift_mono(w.terms, x), rtol=1e-11, atol=1e-11)     # carried state = Psi(x)
+    # and it differs from the linear lifted model on the same inputs (the lifted rows are NOT closed under K)
+    w.model_kind = 0
+    _, _, lin = Oracle(w).rollout(o.lift(x0), u, H=H, want_traj=True)
+    assert not np.allclose(lin[H - 1][: w.n], traj[H - 1][: w.n], rtol=1e-6)
+
+
+def test_relift_reduces_to_textbook_linear_recursion():
+    """If the physical rows of K ignore the lifted features (K[0:n, n:] = 0) the re-lift model is the
+    linear system x' = A x + B_x u with A = K[0:n, 0:n]: x_H = A^H x0 + sum A^k B_x u."""
+    w = _free(W.make("C2", N=8)); w.model_kind = 1
+    w.K = w.K.copy(); w.K[: w.n, w.n:] = 0.0
+    o = Oracle(w)
+    A, Bx = o.K[: w.n, : w.n], o.B[: w.n]
+    x0 = np.array([0.1, -0.05, 0.02, 0.3]); u = np.array([0.7])
+    H = 25
+    _, _, traj = o.rollout(o.lift(x0), u, H=H, want_traj=True)
+    xH = np.linalg.matrix_power(A, H) @ x0 + sum(np.linalg.matrix_power(A, k) @ Bx @ u for k in range(H))
+    assert np.allclose(traj[H - 1][: w.n], xH, rtol=1e-10, atol=1e-12)
+
+
+def test_relift_identity_lift_equals_linear_model():
+    w = _free(W.make("C1", N=8))
+    n = w.n
+    w.d = n; w.K = w.K[:n, :n].copy(); w.B = w.B[:n].copy(); w.terms = w.terms[:n].copy()
+    x0 = np.array([0.1, 0.2, -0.1, 0.05]); u = np.array([-0.4])
+    w.model_kind = 0
+    _, _, a = Oracle(w).rollout(x0, u, H=20, want_traj=True)
+    w.model_kind = 1
+    _, _, b = Oracle(w).rollout(x0, u, H=20, want_traj=True)
+    assert np.array_equal(a, b)

@@ -61,6 +61,8 @@ class Workload:
     rmin: float = 0.0
     rmax: float = 0.0
     inflate: float = 0.0
+    noise_sigma: float = 0.0              # std of the additive prediction noise; 0 = none
+    model_kind: int = 0                   # 0 linear lifted model, 1 re-lift every step
     x_nom: np.ndarray = None
     x_pert: np.ndarray = None             # per-dimension perturbation half-width for tick inputs
     rho: float = 0.0
