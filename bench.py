@@ -97,6 +97,8 @@ def run_reference(args):
     import workloads as W
     from oracle import oracle as O
     w = W.make(args.workload, N=args.N)
+    w.noise_sigma = args.noise
+    w.model_kind = 1 if args.relift else 0
     x0s, uus, ticks = W.tick_inputs(w, args.warmup + args.steps)
     # bounded sample: the first n_ref candidates of the same workload, sized from one probe tick
     n_ref = min(w.N, 1 << 14)
@@ -178,6 +180,9 @@ def main():
     ap.add_argument("--no-latency", action="store_true")
     ap.add_argument("--dump", choices=["lifted", "phys"], default=None,
                     help="measure the trajectory-dump path (mpmi_rollout_batch, SURVEY 8(a) a9) instead of the tick")
+    ap.add_argument("--noise", type=float, default=0.0,
+                    help="std of the additive prediction noise of Alg. 2 l.5 (PAPER.md:150); 0 = the noise-free configs of BASELINE.json")
+    ap.add_argument("--relift", action="store_true", help="re-lift model x' = C(K Psi(x) + B u) instead of the linear lifted model")
     ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
     ap.add_argument("--bounds-scale", type=float, default=1.0,
                     help="scale the safe set (100 = every rollout safe: no early exit, full N*H work)")
@@ -208,6 +213,8 @@ def main():
     w = W.make(args.workload, N=n_per * world)
     if args.bounds_scale != 1.0:
         w = W.generate.scaled_bounds(w, args.bounds_scale)
+    w.noise_sigma = args.noise
+    w.model_kind = 1 if args.relift else 0
     K_, W_ = args.steps, args.warmup
     x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
@@ -362,7 +369,9 @@ def main():
         "vs_baseline": None, "dtype": "f32 (3xTF32 split products, fp32 accumulate)" if info["variant"] == 4 else "f32", "data": "synthetic",
         "config": {"workload": f"{args.workload}: n={w.n} m={w.m} d={w.d} N={n_per}/GPU (+1 user slot) H={w.H}, "
                                f"Philox/grid sampler, calibrated 40% safe (DESIGN.md section 4)"
-                               + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else ""),
+                               + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else "")
+                               + (f", prediction noise sigma={args.noise}" if args.noise else "")
+                               + (", re-lift model" if args.relift else ""),
                    "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
                    "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if world > 1 else "single GPU",
                    "kernel": info},

@@ -51,6 +51,9 @@ typedef enum {
 enum { MPMI_SAMPLER_PHILOX = 0, MPMI_SAMPLER_GRID = 1 };
 enum { MPMI_LIFT_MONO = 0, MPMI_LIFT_RFF = 1 };
 enum { MPMI_DUMP_NONE = 0, MPMI_DUMP_PHYS = 1, MPMI_DUMP_LIFTED = 2 };
+enum { MPMI_MODEL_LINEAR = 0,   /* z' = K z + B u, lifted once, x = z[0:n] (north_star)        */
+       MPMI_MODEL_RELIFT = 1 }; /* x' = C (K Psi(x) + B u): the physical state is re-lifted before every
+                                   step, the literal f(x, u) on states of PAPER.md:132 (G18)     */
 /* mpmi_config.variant: results never depend on these, only speed does */
 enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)                  */
        MPMI_VARIANT_WIDE = 2,           /* 64/D candidates per thread (throughput)            */
@@ -107,6 +110,13 @@ typedef struct {
      * indices [shard_begin, shard_begin + shard_count) of the N (+1) candidates; 0,0 = all of them. */
     int64_t  shard_begin, shard_count;
     int32_t  variant;         /* 0 = automatic; else OR of MPMI_VARIANT_* (benchmark / test knobs)  */
+    /* Additive Gaussian white noise of Algorithm 2 l.5, "x_p <- f(x_p, xi(i)) + z_i":
+     * sigma * eps, eps ~ N(0, I_n), is added to the n physical rows of every predicted state before
+     * isSafe and stays in the state that is carried on; one independent draw per (tick, candidate, step,
+     * dim) from the Philox4x32-10 stream key = (seed_lo, seed_hi ^ 0x6E6F6973), counter = (i, (q << 16) | k,
+     * tick_lo, tick_hi), q = dim / 4, Box-Muller on (w0, w1) and (w2, w3) (G17).  0 = none. */
+    float    noise_sigma;
+    int32_t  model;           /* MPMI_MODEL_* : how f(x, u) is evaluated                            */
     int32_t  reserved;
 } mpmi_config;
 
@@ -134,7 +144,8 @@ typedef struct {
     int32_t  d_pad;           /* internal padded lifted dim (zero rows / columns: exact)            */
     int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = warp-tile FFMA2 (d<=128),
                                  3 = latency kernel, 4 lanes per candidate (d<=32, small N),
-                                 4 = 3xTF32 tcgen05 tensor-core kernel (d_pad = 128)                 */
+                                 4 = 3xTF32 tcgen05 tensor-core kernel (d_pad = 128),
+                                 5 = re-lift kernel (MPMI_MODEL_RELIFT), 6 = affine-in-u kernel       */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;
     int32_t  binning_cells;   /* 0 = candidates walked in index order; else cells of the spatial pre-sort */

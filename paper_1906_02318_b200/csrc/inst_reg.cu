@@ -5,18 +5,25 @@
 #error "compile with -DMPMI_D=8|16|32 -DMPMI_MODE=0|1"
 #endif
 using namespace mpmi;
-#if MPMI_MODE == 0
+#ifndef MPMI_NOISE
+#define MPMI_NOISE 0
+#endif
+#if MPMI_MODE == 0 && !MPMI_NOISE
 #define FN(D) mpmi_pick_reg_##D##_tick
-#else
+#elif !MPMI_NOISE
 #define FN(D) mpmi_pick_reg_##D##_batch
+#elif MPMI_MODE == 0
+#define FN(D) mpmi_pick_regn_##D##_tick
+#else
+#define FN(D) mpmi_pick_regn_##D##_batch
 #endif
 #define FN2(D) FN(D)
 
 template <int M>
 static KernFn pick_p(int P) {
     constexpr int PW = 32 / MPMI_D;                 // wide packing: 2*PW candidates per thread
-    if (P == 1) return rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE>;
-    if (P == PW) return rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE>;
+    if (P == 1) return rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE, (MPMI_NOISE != 0)>;
+    if (P == PW) return rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE, (MPMI_NOISE != 0)>;
     return nullptr;
 }
 KernFn FN2(MPMI_D)(int M, int P) {

@@ -4,19 +4,26 @@
 #error "compile with -DMPMI_D=64|128 -DMPMI_MODE=0|1"
 #endif
 using namespace mpmi;
-#if MPMI_MODE == 0
+#ifndef MPMI_NOISE
+#define MPMI_NOISE 0
+#endif
+#if MPMI_MODE == 0 && !MPMI_NOISE
 #define FN(D) mpmi_pick_tile_##D##_tick
-#else
+#elif !MPMI_NOISE
 #define FN(D) mpmi_pick_tile_##D##_batch
+#elif MPMI_MODE == 0
+#define FN(D) mpmi_pick_tilen_##D##_tick
+#else
+#define FN(D) mpmi_pick_tilen_##D##_batch
 #endif
 #define FN2(D) FN(D)
 
 KernFn FN2(MPMI_D)(int M, int *smem) {
     switch (M) {
-        case 1: *smem = tile_smem_bytes<MPMI_D, 1>(); return rollout_tile_kernel<MPMI_D, 1, MPMI_MODE>;
-        case 2: *smem = tile_smem_bytes<MPMI_D, 2>(); return rollout_tile_kernel<MPMI_D, 2, MPMI_MODE>;
-        case 3: *smem = tile_smem_bytes<MPMI_D, 3>(); return rollout_tile_kernel<MPMI_D, 3, MPMI_MODE>;
-        case 4: *smem = tile_smem_bytes<MPMI_D, 4>(); return rollout_tile_kernel<MPMI_D, 4, MPMI_MODE>;
+        case 1: *smem = tile_smem_bytes<MPMI_D, 1>(); return rollout_tile_kernel<MPMI_D, 1, MPMI_MODE, (MPMI_NOISE != 0)>;
+        case 2: *smem = tile_smem_bytes<MPMI_D, 2>(); return rollout_tile_kernel<MPMI_D, 2, MPMI_MODE, (MPMI_NOISE != 0)>;
+        case 3: *smem = tile_smem_bytes<MPMI_D, 3>(); return rollout_tile_kernel<MPMI_D, 3, MPMI_MODE, (MPMI_NOISE != 0)>;
+        case 4: *smem = tile_smem_bytes<MPMI_D, 4>(); return rollout_tile_kernel<MPMI_D, 4, MPMI_MODE, (MPMI_NOISE != 0)>;
     }
     return nullptr;
 }

@@ -88,15 +88,25 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 }
 
 // kernel tables live in inst_reg.cu / inst_tile.cu, one translation unit per (D, MODE)
-#define MPMI_DECL_REG(D) KernFn mpmi_pick_reg_##D##_tick(int M, int P); KernFn mpmi_pick_reg_##D##_batch(int M, int P);
-#define MPMI_DECL_TILE(D) KernFn mpmi_pick_tile_##D##_tick(int M, int *smem); KernFn mpmi_pick_tile_##D##_batch(int M, int *smem);
+#define MPMI_DECL_REG(D) KernFn mpmi_pick_reg_##D##_tick(int M, int P); KernFn mpmi_pick_reg_##D##_batch(int M, int P); \
+                         KernFn mpmi_pick_regn_##D##_tick(int M, int P); KernFn mpmi_pick_regn_##D##_batch(int M, int P);
+#define MPMI_DECL_TILE(D) KernFn mpmi_pick_tile_##D##_tick(int M, int *smem); KernFn mpmi_pick_tile_##D##_batch(int M, int *smem); \
+                          KernFn mpmi_pick_tilen_##D##_tick(int M, int *smem); KernFn mpmi_pick_tilen_##D##_batch(int M, int *smem);
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
 KernFn mpmi_pick_tc_tick(int *smem, int *threads); KernFn mpmi_pick_tc_batch(int *smem, int *threads);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
-KernFn pick_reg(int D, int M, int P, int mode) {
+KernFn pick_reg(int D, int M, int P, int mode, bool noise) {
     const bool t = mode == MODE_TICK;
+    if (noise) {
+        switch (D) {
+            case 8: return t ? mpmi_pick_regn_8_tick(M, P) : mpmi_pick_regn_8_batch(M, P);
+            case 16: return t ? mpmi_pick_regn_16_tick(M, P) : mpmi_pick_regn_16_batch(M, P);
+            case 32: return t ? mpmi_pick_regn_32_tick(M, P) : mpmi_pick_regn_32_batch(M, P);
+        }
+        return nullptr;
+    }
     switch (D) {
         case 8: return t ? mpmi_pick_reg_8_tick(M, P) : mpmi_pick_reg_8_batch(M, P);
         case 16: return t ? mpmi_pick_reg_16_tick(M, P) : mpmi_pick_reg_16_batch(M, P);
@@ -107,8 +117,13 @@ KernFn pick_reg(int D, int M, int P, int mode) {
 KernFn pick_lat(int D, int M, int R) {
     return D == 8 ? mpmi_pick_lat_8(M, R) : D == 16 ? mpmi_pick_lat_16(M, R) : D == 32 ? mpmi_pick_lat_32(M, R) : nullptr;
 }
-KernFn pick_tile(int D, int M, int mode, int *smem) {
+KernFn pick_tile(int D, int M, int mode, int *smem, bool noise) {
     const bool t = mode == MODE_TICK;
+    if (noise) {
+        if (D == 64) return t ? mpmi_pick_tilen_64_tick(M, smem) : mpmi_pick_tilen_64_batch(M, smem);
+        if (D == 128) return t ? mpmi_pick_tilen_128_tick(M, smem) : mpmi_pick_tilen_128_batch(M, smem);
+        return nullptr;
+    }
     if (D == 64) return t ? mpmi_pick_tile_64_tick(M, smem) : mpmi_pick_tile_64_batch(M, smem);
     if (D == 128) return t ? mpmi_pick_tile_128_tick(M, smem) : mpmi_pick_tile_128_batch(M, smem);
     return nullptr;
@@ -236,6 +251,8 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     if (!cfg->K || !cfg->B || !cfg->u_lo || !cfg->u_hi) return fail(nullptr, MPMI_ERR_INVALID, "null K, B, u_lo or u_hi");
     if (!all_finite(cfg->K, (size_t)d * d) || !all_finite(cfg->B, (size_t)d * m)) return fail(nullptr, MPMI_ERR_INVALID, "non-finite K or B");
     if (!all_finite(cfg->u_lo, m) || !all_finite(cfg->u_hi, m)) return fail(nullptr, MPMI_ERR_INVALID, "non-finite input box");
+    if (!std::isfinite(cfg->noise_sigma) || cfg->noise_sigma < 0.f) return fail(nullptr, MPMI_ERR_INVALID, "noise_sigma must be finite and >= 0");
+    if (cfg->model != MPMI_MODEL_LINEAR && cfg->model != MPMI_MODEL_RELIFT) return fail(nullptr, MPMI_ERR_INVALID, "unknown model kind");
     for (int j = 0; j < m; j++) if (cfg->u_lo[j] > cfg->u_hi[j]) return fail(nullptr, MPMI_ERR_INVALID, "u_lo > u_hi");
     if (cfg->sampler != MPMI_SAMPLER_PHILOX && cfg->sampler != MPMI_SAMPLER_GRID) return fail(nullptr, MPMI_ERR_INVALID, "unknown sampler");
     if (cfg->sampler == MPMI_SAMPLER_GRID) {
@@ -393,6 +410,10 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     }
 
     // ---- kernel choice ------------------------------------------------------------------------------
+    // prediction noise (Alg. 2 l.5) is built into the register and warp-tile kernels; the latency and tensor-core
+    // kernels do not carry it, so sigma != 0 routes around them
+    const bool noise = cfg->noise_sigma != 0.f;
+    dc.noise_sigma = cfg->noise_sigma; dc.model = cfg->model;
     if (D <= 32) {
         c->variant = 1;
         const int Pmax = 32 / D;
@@ -404,10 +425,10 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         c->cand_per_block = 2 * c->P * c->block;
         c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
         c->smem = 0;
-        c->k_tick = pick_reg(D, M, c->P, MODE_TICK);
-        c->k_batch = pick_reg(D, M, c->P, MODE_BATCH);
+        c->k_tick = pick_reg(D, M, c->P, MODE_TICK, noise);
+        c->k_batch = pick_reg(D, M, c->P, MODE_BATCH, noise);
         // paper-scale candidate sets: 4 lanes per candidate (rollout_lat.cuh) shorten the dependent chain
-        const bool lat = (cfg->variant & MPMI_VARIANT_LATENCY) || (!(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE)) && sc <= kLatMaxCand);
+        const bool lat = !noise && ((cfg->variant & MPMI_VARIANT_LATENCY) || (!(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE)) && sc <= kLatMaxCand));
         if (lat && !c->binning) {
             // rows per lane: 2 (D/2 lanes per candidate) while that still leaves SMs short of warps, else 4
             const long long warps_r4 = sc * (D / 4) / 32;
@@ -420,7 +441,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     } else {
         // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)
         // unless the caller asks for the FP32 SIMT tile kernel; d = 64 stays on the SIMT tile kernel
-        const bool tensor = D == 128 && !(cfg->variant & MPMI_VARIANT_NO_TENSOR);
+        const bool tensor = D == 128 && !noise && !(cfg->variant & MPMI_VARIANT_NO_TENSOR);
         c->P = 1;
         if (tensor) {
             c->variant = 4;
@@ -431,8 +452,8 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         } else {
             c->variant = 2;
             c->block = kTileThreads; c->cand_per_block = kTileNC;
-            c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem);
-            c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem);
+            c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem, noise);
+            c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem, noise);
         }
         c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
         if (c->k_tick) {

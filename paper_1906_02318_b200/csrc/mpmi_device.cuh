@@ -34,6 +34,8 @@ struct DevCfg {
     const float *Bpad;              // device: D*4 row-major padded B
     const uint8_t *terms;           // device: D*4 lift factor codes (MONO)
     const float *W, *b;             // device: RFF tables
+    float noise_sigma;              // std of the additive prediction noise (Alg. 2 l.5); 0 = none
+    int model;                      // MPMI_MODEL_*
 };
 
 // Cross-block selection state; reset by the block that finalises the tick.
@@ -100,6 +102,24 @@ __device__ __forceinline__ void sample_u(const DevCfg &cfg, long long gi, unsign
                 u[j] = v;
             }
         }
+    }
+}
+
+// Algorithm 2 l.5 noise z_i (DESIGN G17): four standard normals for the original physical
+// dims 4q..4q+3 of candidate gi at step k, Box-Muller on the Philox words (w0, w1) and (w2, w3).
+__device__ __forceinline__ void noise4(const DevCfg &cfg, long long gi, int k, int q, unsigned long long tick, float (&g)[4]) {
+    unsigned w[4];
+    philox4x32_10((unsigned)gi, ((unsigned)q << 16) | (unsigned)k, (unsigned)tick, (unsigned)(tick >> 32),
+                  cfg.seed_lo, cfg.seed_hi ^ 0x6E6F6973u, w);
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        const float u1 = __fmaf_rn(__uint2float_rn(w[2 * h] >> 8), 0x1p-24f, 0x1p-24f);   // ((w >> 8) + 1) 2^-24, exact
+        const float u2 = __uint2float_rn(w[2 * h + 1] >> 8) * 0x1p-23f;                    // 2 u2: angle in units of pi
+        const float r = sqrtf(-2.0f * logf(u1));
+        float sn, cs;
+        sincospif(u2, &sn, &cs);
+        g[2 * h] = r * cs;
+        g[2 * h + 1] = r * sn;
     }
 }
 

@@ -46,7 +46,7 @@ __device__ __forceinline__ bool safe_check(const DevCfg &cfg, const float (&x)[N
 template <int D, int P>
 constexpr int reg_min_blocks() { return (D * P >= 32) ? 3 : 4; }
 
-template <int D, int M, int P, int MODE>
+template <int D, int M, int P, int MODE, bool NOISE = false>
 __global__ void __launch_bounds__(kRegBlock, reg_min_blocks<D, P>())
 rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     constexpr int S = 2 * P;                 // candidates per thread
@@ -165,6 +165,31 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
             for (int r = 0; r < D; r++) z[p][r] = acc[p][r];
 
+        if (NOISE) {
+            // Algorithm 2 l.5: x_p <- f(x_p, xi(i)) + z_i: sigma * eps on the physical rows, before isSafe
+#pragma unroll
+            for (int s = 0; s < S; s++) {
+                const long long gi = (MODE == MODE_TICK ? cfg.shard_begin : 0) + li[s];
+                float g[NB];                                   // eps of the ORIGINAL dims
+#pragma unroll
+                for (int q = 0; 4 * q < NB; q++) {
+                    float g4[4] = {0.f, 0.f, 0.f, 0.f};
+                    if (4 * q < cfg.n) noise4(cfg, gi, k, q, tick, g4);
+#pragma unroll
+                    for (int e = 0; e < 4; e++) if (4 * q + e < NB) g[4 * q + e] = g4[e];
+                }
+#pragma unroll
+                for (int j = 0; j < NB; j++) {
+                    if (j < cfg.n) {                           // internal dim j = original dim perm[j]
+                        float e = 0.f;
+#pragma unroll
+                        for (int p = 0; p < NB; p++) e = ((int)cfg.perm[j] == p) ? g[p] : e;
+                        if (s & 1) z[s >> 1][j].y = __fmaf_rn(cfg.noise_sigma, e, z[s >> 1][j].y);
+                        else       z[s >> 1][j].x = __fmaf_rn(cfg.noise_sigma, e, z[s >> 1][j].x);
+                    }
+                }
+            }
+        }
         bool was_alive[S];
 #pragma unroll
         for (int s = 0; s < S; s++) {

@@ -25,7 +25,7 @@ constexpr int kTileThreadsT = kTileWarps * 32;
 template <int D, int M>
 constexpr int tile_smem_bytes() { return ((D + M) * D + kTileWarps * (D + M) * kTileWC) * 4; }
 
-template <int D, int M, int MODE>
+template <int D, int M, int MODE, bool NOISE = false>
 __global__ void __launch_bounds__(kTileThreadsT, 1)
 rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     constexpr int WC = kTileWC;
@@ -154,6 +154,24 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
             }
             __syncwarp();
 
+            if (NOISE) {
+                // Algorithm 2 l.5: + z_i: sigma * eps on the physical rows of candidate `col`, before isSafe
+                if (lane < WC) {
+                    const long long gi = (MODE == MODE_TICK ? cfg.shard_begin : 0) + li;
+                    for (int q = 0; 4 * q < cfg.n; q++) {
+                        float g[4];
+                        noise4(cfg, gi, k, q, tick, g);
+                        for (int j = 0; j < cfg.n; j++) {            // internal dim j = original dim perm[j]
+                            const int p = cfg.perm[j];
+                            if ((p >> 2) == q) {
+                                const float e = (p & 3) == 0 ? g[0] : (p & 3) == 1 ? g[1] : (p & 3) == 2 ? g[2] : g[3];
+                                zw[j * WC + col] = __fmaf_rn(cfg.noise_sigma, e, zw[j * WC + col]);
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+            }
             float x[NB];
 #pragma unroll
             for (int j = 0; j < NB; j++) x[j] = j < nphys ? zw[j * WC + col] : 0.f;

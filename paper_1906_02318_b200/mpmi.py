@@ -46,7 +46,7 @@ class _Config(C.Structure):
                 ("sampler", C.c_int32), ("grid_counts", C.c_void_p), ("seed", C.c_uint64),
                 ("include_user", C.c_int32), ("lift", _Lift), ("safe", _Safe), ("device", C.c_int32),
                 ("shard_begin", C.c_int64), ("shard_count", C.c_int64), ("variant", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("noise_sigma", C.c_float), ("model", C.c_int32), ("reserved", C.c_int32)]
 
 
 class Result(C.Structure):
@@ -146,6 +146,7 @@ class Context:
                        int(g("annulus", 0)), int(g("ix", 0)), int(g("iy", 1)), float(g("cx", 0.0)), float(g("cy", 0.0)),
                        float(g("rmin", 0.0)), float(g("rmax", 0.0)), float(g("inflate", 0.0)))
         c.device, c.shard_begin, c.shard_count, c.variant = device, int(shard[0]), int(shard[1]), variant
+        c.noise_sigma, c.model = float(g("noise_sigma", 0.0)), int(g("model_kind", 0))
         h = C.c_void_p()
         rc = self._lib.mpmi_create(C.byref(c), C.byref(h))
         if rc != OK:

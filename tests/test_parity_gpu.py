@@ -346,3 +346,48 @@ def test_full_size_sampled(mp, name):
             ok = g_steps[: 1 << 15] == H
             if ok.any() and us != H:
                 assert dd[ok].min() >= r["dist"] - 1e-6
+
+
+# ------------------------------------------------------------------ NEXT-2: prediction noise (Alg. 2 l.5) ----------
+NOISE_SIGMA = {"C1": 0.05, "C2": 0.01, "C4": 0.02, "C5": 0.01}
+
+
+@pytest.mark.parametrize("name,N,per_cand_x0", [("C1", 900, False), ("C2", 1300, False), ("C4", 777, False),
+                                                ("C4", 1030, True), ("C5", 600, False)])
+def test_noise_rollout_batch_parity(mp, name, N, per_cand_x0):
+    """x_p <- f(x_p, xi) + z_i with Gaussian z_i: same counter-based draws on both sides, T1 / T2."""
+    w = W.make(name, N=N); w.noise_sigma = NOISE_SIGMA[name]; w.seed = 0xABCDEF0123
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    assert ctx.info()["variant"] in (1, 2)                       # register / warp-tile kernel: the ones that carry noise
+    rng = np.random.default_rng(5)
+    U = rng.uniform(w.u_lo, w.u_hi, (N, w.m)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, N if per_cand_x0 else 1)
+    H, tick = w.H, (3 << 32) | 41
+    traj = torch.full((H, w.d, N), 7.0, dtype=torch.float32, device="cuda")
+    steps = torch.empty(N, dtype=torch.int32, device="cuda")
+    dU, dX = _dev(U), _dev(x0s)
+    ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), x0s.shape[0], N, H, mp.DUMP_LIFTED, traj.data_ptr(),
+                      steps.data_ptr(), 0, tick=tick)
+    torch.cuda.synchronize()
+    g_steps = steps.cpu().numpy(); g_traj = traj.cpu().numpy()
+    r_steps, r_marg, r_traj = o.rollout_batch(U, x0s, want_traj=True, tick=tick)
+    bad, nrobust = check_flags(g_steps, r_steps, r_marg, H)
+    assert len(bad) == 0, (bad[:5], g_steps[bad[:5]], r_steps[bad[:5]], r_marg[bad[:5]])
+    assert nrobust > 0.9 * N
+    w0 = W.make(name, N=N); w0.seed = w.seed                      # the noise really changes the outcome
+    q_steps, _, _ = _oracle(w0).rollout_batch(U, x0s, tick=tick)
+    assert (q_steps != r_steps).any()
+    worst = 0.0
+    for i in range(N):
+        e = min(r_steps[i] + 1, g_steps[i] + 1, H)
+        worst = max(worst, traj_rel_err(g_traj[:, :, i], r_traj[i], e))
+    assert worst <= TRAJ_RTOL, worst
+
+
+@pytest.mark.parametrize("name,N", [("C2", 10000), ("C4", 1 << 15), ("C5", 1500)])
+def test_noise_tick_parity(mp, name, N):
+    """whole tick with prediction noise: T3 selection against the oracle on the same draws (binned order at C4)."""
+    w = W.make(name, N=N); w.noise_sigma = NOISE_SIGMA[name]
+    rate, branches = _tick_compare(mp, w, 12 if name != "C5" else 6)
+    assert rate >= 0.9, rate
