@@ -35,6 +35,9 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.45: SMs x FP32 lanes
 
 
 def _flop_per_sample_step(w):
+    if getattr(w, "model_kind", 0) == 1:                # re-lift model: n physical rows + the lift itself (cos / sin counted as 1)
+        lift = 3.0 * w.d if w.lift_kind == 0 else (2.0 * w.n + 2.0) * (w.d - w.n)
+        return 2.0 * w.n * (w.d + w.m) + lift
     return 2.0 * w.d * (w.d + w.m)                      # dense K and B, nothing discounted
 
 
@@ -341,7 +344,8 @@ def main():
         roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
-                    "kernel": "rollout_reg_kernel" if info["variant"] == 1 else "rollout_tile_kernel",
+                    "kernel": {1: "rollout_reg_kernel", 2: "rollout_tile_kernel", 3: "rollout_lat_kernel", 5: "rollout_relift_kernel",
+                               6: "rollout_affine_kernel"}.get(info["variant"], "?"),
                     "nominal_frac": nominal_frac}
 
     if rank != 0:

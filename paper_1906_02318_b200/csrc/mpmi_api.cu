@@ -94,6 +94,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
                           KernFn mpmi_pick_tilen_##D##_tick(int M, int *smem); KernFn mpmi_pick_tilen_##D##_batch(int M, int *smem);
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
+KernFn mpmi_pick_relift(int n, int mode);
 KernFn mpmi_pick_tc_tick(int *smem, int *threads); KernFn mpmi_pick_tc_batch(int *smem, int *threads);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
@@ -414,7 +415,14 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     // kernels do not carry it, so sigma != 0 routes around them
     const bool noise = cfg->noise_sigma != 0.f;
     dc.noise_sigma = cfg->noise_sigma; dc.model = cfg->model;
-    if (D <= 32) {
+    if (cfg->model == MPMI_MODEL_RELIFT) {
+        // x' = C (K Psi(x) + B u): one thread per candidate, only the physical rows of the model (rollout_relift.cuh)
+        c->variant = 5;
+        c->P = 1; c->block = 128; c->cand_per_block = 128; c->smem = 0;
+        c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
+        c->k_tick = mpmi_pick_relift(n, MODE_TICK);
+        c->k_batch = mpmi_pick_relift(n, MODE_BATCH);
+    } else if (D <= 32) {
         c->variant = 1;
         const int Pmax = 32 / D;
         // enough warps to give every SM sub-partition two warps at the wide packing?  else 2 cand/thread

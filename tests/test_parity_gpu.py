@@ -391,3 +391,58 @@ def test_noise_tick_parity(mp, name, N):
     w = W.make(name, N=N); w.noise_sigma = NOISE_SIGMA[name]
     rate, branches = _tick_compare(mp, w, 12 if name != "C5" else 6)
     assert rate >= 0.9, rate
+
+
+# ------------------------------------------------------------------ NEXT-3: re-lift model x' = C(K Psi(x) + B u) ----
+def _relift(name, N, bounds=None, sigma=0.0):
+    w = W.make(name, N=N)
+    if name == "C3":
+        side = int(round(N ** 0.5)); w.N = side * side; w.grid_counts = np.array([side, side], np.int32)
+    if bounds is not None:
+        w = G.scaled_bounds(w, bounds)
+    w.model_kind = 1; w.noise_sigma = sigma
+    return w
+
+
+@pytest.mark.parametrize("name,N,per_cand_x0,bounds,sigma", [("C2", 1300, False, None, 0.0), ("C1", 700, True, None, 0.0),
+                                                             ("C4", 900, False, None, 0.0), ("C4", 1100, True, None, 0.02),
+                                                             ("C5", 500, False, 0.25, 0.0)])
+def test_relift_rollout_batch_parity(mp, name, N, per_cand_x0, bounds, sigma):
+    """T1 / T2 for the re-lift model (polynomial, trig-product and RFF lifts), physical and lifted dumps, NaN tail."""
+    w = _relift(name, N, bounds, sigma)
+    w.sampler = 0; w.grid_counts = None
+    o = _oracle(w)
+    ctx = mp.Context(w)
+    assert ctx.info()["variant"] == 5
+    rng = np.random.default_rng(23)
+    U = rng.uniform(w.u_lo, w.u_hi, (N, w.m)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, N if per_cand_x0 else 1)
+    H, tick = w.H, 17
+    r_steps, r_marg, r_traj = o.rollout_batch(U, x0s, want_traj=True, tick=tick)
+    assert 0.02 < (r_steps == H).mean() < 0.98
+    for kind, J in ((mp.DUMP_LIFTED, w.d), (mp.DUMP_PHYS, w.n)):
+        traj = torch.full((H, J, N), 7.0, dtype=torch.float32, device="cuda")
+        steps = torch.empty(N, dtype=torch.int32, device="cuda")
+        safe = torch.empty(N, dtype=torch.uint8, device="cuda")
+        dU, dX = _dev(U), _dev(x0s)
+        ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), x0s.shape[0], N, H, kind, traj.data_ptr(),
+                          steps.data_ptr(), safe.data_ptr(), tick=tick)
+        torch.cuda.synchronize()
+        g_steps = steps.cpu().numpy(); g_traj = traj.cpu().numpy()
+        bad, nrobust = check_flags(g_steps, r_steps, r_marg, H)
+        assert len(bad) == 0, (bad[:5], g_steps[bad[:5]], r_steps[bad[:5]], r_marg[bad[:5]])
+        assert nrobust > 0.9 * N
+        assert np.array_equal(safe.cpu().numpy(), (g_steps == H).astype(np.uint8))
+        worst = 0.0
+        for i in range(N):
+            e = min(r_steps[i] + 1, g_steps[i] + 1, H); e_gpu = min(g_steps[i] + 1, H)
+            worst = max(worst, traj_rel_err(g_traj[:, :, i], r_traj[i][:, :J], e))
+            assert np.all(np.isfinite(g_traj[:e_gpu, :, i])) and np.all(np.isnan(g_traj[e_gpu:, :, i]))
+        assert worst <= TRAJ_RTOL, (kind, worst)
+
+
+@pytest.mark.parametrize("name,N,bounds", [("C2", 10000, None), ("C3", 10000, None), ("C4", 1 << 15, None), ("C5", 3000, 0.25)])
+def test_relift_tick_parity(mp, name, N, bounds):
+    w = _relift(name, N, bounds)
+    rate, branches = _tick_compare(mp, w, 12)
+    assert rate >= 0.9, rate
