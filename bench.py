@@ -186,6 +186,8 @@ def main():
     ap.add_argument("--noise", type=float, default=0.0,
                     help="std of the additive prediction noise of Alg. 2 l.5 (PAPER.md:150); 0 = the noise-free configs of BASELINE.json")
     ap.add_argument("--relift", action="store_true", help="re-lift model x' = C(K Psi(x) + B u) instead of the linear lifted model")
+    ap.add_argument("--affine", action="store_true",
+                    help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
     ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
     ap.add_argument("--bounds-scale", type=float, default=1.0,
                     help="scale the safe set (100 = every rollout safe: no early exit, full N*H work)")
@@ -223,7 +225,7 @@ def main():
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
     begin, count = shard_plan(w.N, 1, world, rank)             # the injected u_user (index N) goes to the last rank
     ctx = mp.Context(w, device=local, shard=(begin, count) if world > 1 else (0, 0),
-                     variant=mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0)
+                     variant=(mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0))
     info = ctx.info()
     stream = torch.cuda.current_stream().cuda_stream
     if args.dump:
@@ -316,7 +318,7 @@ def main():
             c2.close()
 
     # ---- roofline of the dominant (only) kernel: plain FP32 FMA arithmetic
-    flop = _flop_per_sample_step(w)
+    flop = _flop_per_sample_step(w) if info["variant"] != 6 else 2.0 * w.n * w.m      # affine path: n*m FMAs per sample-step
     achieved = n_exec / world * flop / (total_ms * 1e-3) / 1e12            # per GPU
     traffic = None
     tj = os.path.join(ROOT, "profiles", "roofline_traffic.csv")     # ncu --set full, dram bytes per launch
@@ -375,7 +377,8 @@ def main():
                                f"Philox/grid sampler, calibrated 40% safe (DESIGN.md section 4)"
                                + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else "")
                                + (f", prediction noise sigma={args.noise}" if args.noise else "")
-                               + (", re-lift model" if args.relift else ""),
+                               + (", re-lift model" if args.relift else "")
+                               + (", affine-in-u fast path (NEXT-4: separate metric, 2nm flop per sample-step)" if info["variant"] == 6 else ""),
                    "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
                    "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if world > 1 else "single GPU",
                    "kernel": info},

@@ -26,6 +26,13 @@ struct mpmi_ctx {
     int block = 128, cand_per_block = 0;              // launch geometry of the tick kernel
     int bblock = 128, bcand_per_block = 0;            // launch geometry of the batch kernel
     KernFn k_tick = nullptr, k_batch = nullptr;
+    int bsmem = 0;                                    // dynamic shared memory of the batch kernel
+    bool bpersistent = false;                         // batch kernel is a persistent one-CTA-per-SM kernel
+    // affine-in-u fast path (rollout_affine.cuh)
+    bool affine = false;
+    KernFn k_base = nullptr, k_batch_aff = nullptr;
+    float *d_affA = nullptr, *d_affG = nullptr;
+    cudaGraphNode_t n_base = nullptr;
     float *d_KTa = nullptr, *d_W = nullptr, *d_b = nullptr;
     uint8_t *d_terms = nullptr;
     TickState *d_state = nullptr;
@@ -95,6 +102,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
 KernFn mpmi_pick_relift(int n, int mode);
+KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
 KernFn mpmi_pick_tc_tick(int *smem, int *threads); KernFn mpmi_pick_tc_batch(int *smem, int *threads);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
@@ -136,17 +144,24 @@ bool all_finite(const float *p, size_t n) {
 }
 
 void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
-    const bool batch = fn == c->k_batch;
-    const int cpb = batch ? c->bcand_per_block : c->cand_per_block, block = batch ? c->bblock : c->block;
+    const bool batch = fn == c->k_batch, aff_batch = fn == c->k_batch_aff && fn != nullptr;
+    const int cpb = aff_batch ? 256 : batch ? c->bcand_per_block : c->cand_per_block;
+    const int block = aff_batch ? 256 : batch ? c->bblock : c->block;
+    const int smem = aff_batch ? a0.H * (1 + c->dc.m) * c->dc.aff_np * 4 : batch ? c->bsmem : c->smem;
     long long blocks = (ncand + cpb - 1) / cpb;
     if (blocks < 1) blocks = 1;
     KArgs a = a0;
-    if (c->variant == 2 || c->variant == 4) {    // persistent warp-tile / tensor-core kernel: one CTA per SM
+    const bool persistent = !aff_batch && (batch ? c->bpersistent : c->variant == 2 || c->variant == 4);
+    if (persistent) {                            // persistent warp-tile / tensor-core kernel: one CTA per SM
         if (blocks > c->sm_count) blocks = c->sm_count;
         a.st = c->d_state; a.work = &c->d_state->work;
     }
     void *args[2] = {(void *)&c->dc, (void *)&a};
-    cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)c->smem, s);
+    cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)smem, s);
+}
+void launch_base(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {      // a_k = C K^k Psi(x_t) of the affine path
+    void *args[2] = {(void *)&c->dc, (void *)&a};
+    cudaLaunchKernel((const void *)c->k_base, dim3(1), dim3((unsigned)c->dc.D), args, 0, s);
 }
 
 // one tick on stream s: [cell histogram + scan, scatter] (large Philox sets only) -> fused tick kernel
@@ -161,6 +176,7 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         bin_scatter_kernel<<<grid, 256, 0, s>>>(c->dc, b);
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
+    if (c->affine) launch_base(c, a, s);
     launch(c, c->k_tick, c->dc.shard_count, a, s);
 }
 
@@ -176,6 +192,11 @@ void tick_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
     p->func = (void *)c->k_tick; p->gridDim = dim3(c->tick_grid); p->blockDim = dim3((unsigned)c->block);
     p->sharedMemBytes = (unsigned)c->smem; p->kernelParams = args;
+}
+void base_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
+    p->func = (void *)c->k_base; p->gridDim = dim3(1); p->blockDim = dim3((unsigned)c->dc.D); p->kernelParams = args;
 }
 void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
@@ -204,8 +225,15 @@ int build_graph(mpmi_ctx *c) {
         CU(c, cudaGraphAddKernelNode(&c->n_scatter, c->graph, &c->n_hist, 1, &p));
         dep = c->n_scatter;
     }
+    cudaGraphNode_t deps[2]; int ndep = 0;
+    if (dep) deps[ndep++] = dep;
+    if (c->affine) {                             // independent of the binning nodes: runs beside them
+        base_node_params(c, &p, args);
+        CU(c, cudaGraphAddKernelNode(&c->n_base, c->graph, nullptr, 0, &p));
+        deps[ndep++] = c->n_base;
+    }
     tick_node_params(c, &p, args);
-    CU(c, cudaGraphAddKernelNode(&c->n_tick, c->graph, dep ? &dep : nullptr, dep ? 1 : 0, &p));
+    CU(c, cudaGraphAddKernelNode(&c->n_tick, c->graph, ndep ? deps : nullptr, ndep, &p));
     CU(c, cudaGraphInstantiate(&c->exec, c->graph, 0));
     return MPMI_OK;
 }
@@ -235,6 +263,7 @@ void mpmi_destroy(mpmi_ctx *c) {
     if (c->graph) cudaGraphDestroy(c->graph);
     cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
     cudaFree(c->d_state);
+    cudaFree(c->d_affA); cudaFree(c->d_affG);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_res);
     delete c;
@@ -469,6 +498,41 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
         }
     }
+    c->bsmem = c->smem;
+    c->bpersistent = c->variant == 2 || c->variant == 4;
+    if ((cfg->variant & MPMI_VARIANT_AFFINE) && cfg->model == MPMI_MODEL_LINEAR && !noise && c->k_tick && c->k_batch) {
+        // x_k = a_k + G_k u: tabulate G_k = C S_k B, S_k = sum_{i<k} K^i, in FP64 (T_1 = B, T_{k+1} = K T_k + B)
+        const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16, Hh = cfg->H;
+        const size_t aff_smem = (size_t)Hh * (1 + m) * NPn * sizeof(float);
+        if (aff_smem <= 200 * 1024) {
+            std::vector<double> T((size_t)d * m), Tn((size_t)d * m);
+            std::vector<float> G((size_t)Hh * m * NPn, 0.f);
+            for (int r = 0; r < d; r++) for (int j = 0; j < m; j++) T[(size_t)r * m + j] = cfg->B[(size_t)r * m + j];
+            for (int k = 0; k < Hh; k++) {
+                for (int j = 0; j < m; j++)
+                    for (int q = 0; q < n; q++) G[((size_t)k * m + j) * NPn + q] = (float)T[(size_t)perm[q] * m + j];
+                for (int r = 0; r < d; r++)
+                    for (int j = 0; j < m; j++) {
+                        double sacc = cfg->B[(size_t)r * m + j];
+                        for (int q = 0; q < d; q++) sacc += (double)cfg->K[(size_t)r * d + q] * T[(size_t)q * m + j];
+                        Tn[(size_t)r * m + j] = sacc;
+                    }
+                T.swap(Tn);
+            }
+            CUC(cudaMalloc(&c->d_affG, G.size() * sizeof(float)));
+            CUC(cudaMemcpy(c->d_affG, G.data(), G.size() * sizeof(float), cudaMemcpyHostToDevice));
+            CUC(cudaMalloc(&c->d_affA, (size_t)Hh * NPn * sizeof(float)));
+            CUC(cudaMemset(c->d_affA, 0, (size_t)Hh * NPn * sizeof(float)));
+            dc.aff_g = c->d_affG; dc.aff_a = c->d_affA; dc.aff_np = NPn;
+            c->affine = true; c->variant = 6;
+            c->k_base = mpmi_pick_affine_base(D);
+            c->k_tick = mpmi_pick_affine(NPn, MODE_TICK);
+            c->k_batch_aff = mpmi_pick_affine(NPn, MODE_BATCH);
+            c->block = 256; c->cand_per_block = 256; c->smem = (int)aff_smem;
+            CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+            CUC(cudaFuncSetAttribute((const void *)c->k_batch_aff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+        }
+    }
     if (!c->k_tick || !c->k_batch) { c->err = "no kernel for this (d, m)"; return bail(MPMI_ERR_UNSUPPORTED); }
     cudaFuncAttributes fa;
     CUC(cudaFuncGetAttributes(&fa, (const void *)c->k_tick));
@@ -488,7 +552,7 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
     if ((c->variant == 2 || c->variant == 4) && o->blocks > c->sm_count) o->blocks = c->sm_count;
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
-    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = c->binning ? 3 : 1; o->uses_graph = 1;
+    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0); o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;
     o->ncand_local = c->dc.shard_count;
     return MPMI_OK;
@@ -516,6 +580,10 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
         CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_hist, &p));
         bin_node_params(c, true, &p, args);
         CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_scatter, &p));
+    }
+    if (c->affine) {
+        base_node_params(c, &p, args);
+        CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_base, &p));
     }
     tick_node_params(c, &p, args);
     CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_tick, &p));
@@ -599,7 +667,12 @@ int mpmi_rollout_batch(mpmi_ctx *c, const float *d_U, const float *d_X0, int64_t
     a.x0 = d_X0; a.u_user = nullptr; a.tick_val = tick;
     a.U = d_U; a.x0_count = x0_count; a.ncand = Ncand; a.H = H; a.dump_kind = dump_kind;
     a.traj = d_traj; a.steps = d_steps; a.safe = d_safe;
-    launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream);
+    if (c->affine && dump_kind != MPMI_DUMP_LIFTED && x0_count == 1 && H <= c->dc.H) {
+        launch_base(c, a, (cudaStream_t)stream);                 // physical states only, shared x0: the affine path applies
+        launch(c, c->k_batch_aff, Ncand, a, (cudaStream_t)stream);
+    } else {
+        launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream);
+    }
     CU(c, cudaGetLastError());
     return MPMI_OK;
 }

@@ -36,6 +36,10 @@ struct DevCfg {
     const float *W, *b;             // device: RFF tables
     float noise_sigma;              // std of the additive prediction noise (Alg. 2 l.5); 0 = none
     int model;                      // MPMI_MODEL_*
+    // affine-in-u fast path (rollout_affine.cuh): x_k = a_k + G_k u
+    float *aff_a;                   // device: H x aff_np, written per tick by affine_base_kernel
+    const float *aff_g;             // device: H x m x aff_np, from mpmi_create (FP64 -> fp32)
+    int aff_np;                     // padded physical dim: 4, 8 or 16
 };
 
 // Cross-block selection state; reset by the block that finalises the tick.

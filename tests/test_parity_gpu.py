@@ -446,3 +446,64 @@ def test_relift_tick_parity(mp, name, N, bounds):
     w = _relift(name, N, bounds)
     rate, branches = _tick_compare(mp, w, 12)
     assert rate >= 0.9, rate
+
+
+# ------------------------------------------------------------------ NEXT-4: affine-in-u fast path -------------------
+@pytest.mark.parametrize("name,N", [("C1", 1100), ("C2", 1300), ("C4", 900), ("C5", 700)])
+def test_affine_rollout_batch_parity(mp, name, N):
+    """x_k = a_k + G_k u must reproduce the step-by-step oracle: physical trajectories, flags (T2), NaN tail;
+    a lifted dump or per-candidate x0 falls back to the full rollout kernel inside the same context."""
+    w = W.make(name, N=N)
+    o = _oracle(w)
+    ctx = mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE)
+    assert ctx.info()["variant"] == 6
+    rng = np.random.default_rng(31)
+    U = rng.uniform(w.u_lo, w.u_hi, (N, w.m)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, 1)
+    H = w.H
+    r_steps, r_marg, r_traj = o.rollout_batch(U, x0s, want_traj=True)
+    for kind, J in ((mp.DUMP_PHYS, w.n), (mp.DUMP_LIFTED, w.d)):
+        traj = torch.full((H, J, N), 7.0, dtype=torch.float32, device="cuda")
+        steps = torch.empty(N, dtype=torch.int32, device="cuda")
+        dU, dX = _dev(U), _dev(x0s)
+        ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), 1, N, H, kind, traj.data_ptr(), steps.data_ptr(), 0)
+        torch.cuda.synchronize()
+        g_steps = steps.cpu().numpy(); g_traj = traj.cpu().numpy()
+        bad, nrobust = check_flags(g_steps, r_steps, r_marg, H)
+        assert len(bad) == 0, (kind, bad[:5], g_steps[bad[:5]], r_steps[bad[:5]], r_marg[bad[:5]])
+        assert nrobust > 0.9 * N
+        for i in range(N):
+            e = min(r_steps[i] + 1, g_steps[i] + 1, H); e_gpu = min(g_steps[i] + 1, H)
+            ref = r_traj[i][:e, :J]
+            scale = np.maximum(np.linalg.norm(r_traj[i][:e], axis=1), 1e-3)[:, None]      # T1 scale: the lifted state's norm
+            assert np.all(np.abs(g_traj[:e, :, i] - ref) <= TRAJ_RTOL * scale)
+            assert np.all(np.isfinite(g_traj[:e_gpu, :, i])) and np.all(np.isnan(g_traj[e_gpu:, :, i]))
+
+
+@pytest.mark.parametrize("name,N", [("C1", 1024), ("C2", 10000), ("C3", 10000), ("C4", 1 << 15), ("C5", 2048)])
+def test_affine_tick_parity(mp, name, N):
+    """T3 through the affine path, and the same winner as the full rollout kernel on every tick."""
+    w = _small(name, N) if name == "C3" else W.make(name, N=N)
+    o = _oracle(w)
+    aff = mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE)
+    full = mp.Context(w)
+    assert aff.info()["variant"] == 6 and full.info()["variant"] != 6
+    x0s, uus, ticks = W.tick_inputs(w, 16)
+    exact = 0
+    for x0, uu, t in zip(x0s, uus, ticks):
+        ref = o.step(x0, uu, int(t), detail=True)
+        r = aff.step_sync(x0, uu, int(t)).as_dict(w.m)
+        ok, ex, why = accept_selection(r, ref, w.H)
+        assert ok, (why, r, {k: ref[k] for k in ("index", "safe", "steps", "dist")})
+        exact += ex
+        f = full.step_sync(x0, uu, int(t)).as_dict(w.m)
+        if (ref["margin_all"] > MARGIN).all():
+            assert (r["index"], r["safe"], r["steps"], r["n_safe"], r["n_exec"]) == (f["index"], f["safe"], f["steps"], f["n_safe"], f["n_exec"])
+    assert exact >= 15
+
+
+def test_affine_flag_ignored_with_noise_or_relift(mp):
+    w = W.make("C2", N=2000); w.noise_sigma = 0.01
+    assert mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE).info()["variant"] == 1
+    w = W.make("C2", N=2000); w.model_kind = 1
+    assert mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE).info()["variant"] == 5
