@@ -196,7 +196,8 @@ int mpmi_shard_finalize(mpmi_ctx *ctx, const mpmi_partial *d_partials, int32_t G
  *   H       horizon for this call (<= 65535)
  *   d_traj  device or NULL; dump_kind PHYS: H*n*Ncand floats, LIFTED: H*d*Ncand floats, laid out
  *           traj[(k*J + j)*Ncand + i] = component j of z_{k+1} of candidate i (candidate fastest);
- *           entries after a candidate's first violating state are NaN
+ *           entries after a candidate's first violating state are NaN; with MPMI_MODEL_RELIFT a LIFTED
+ *           dump holds the carried state Psi(x_{k+1}); with noise the dumped state includes it
  *   d_steps device, Ncand int32: safe predicted states before the first violation (H <=> safe)
  *   d_safe  device or NULL, Ncand bytes: 1 iff steps == H
  * Asynchronous on cuda_stream. */
