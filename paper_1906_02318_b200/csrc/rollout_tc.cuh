@@ -37,7 +37,11 @@ namespace mpmi {
 constexpr int kTcD = 128;                         // padded lifted dim
 constexpr int kTcKD = 136;                        // contraction length: 128 state + 8 input columns (m <= 4, zero padded)
 constexpr int kTcTile = 128;                      // candidates per tile = TMEM lanes
-constexpr int kTcStateWarps = 8;
+#ifndef MPMI_TC_STATE_WARPS
+#define MPMI_TC_STATE_WARPS 8
+#endif
+constexpr int kTcStateWarps = MPMI_TC_STATE_WARPS;             // 4 lane quadrants x (2 or 4) column groups
+constexpr int kTcCols = 128 / (kTcStateWarps / 4);         // state columns per state-warp thread
 constexpr int kTcThreads = (kTcStateWarps + 1) * 32;
 constexpr int kTcLBO = 128;                       // bytes between 16-byte K chunks (core matrices contiguous along K)
 constexpr int kTcSBO = (kTcKD / 4) * 128;         // bytes between 8-row groups
@@ -223,10 +227,10 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         __syncwarp();
     } else {
         // ================= state warps: thread = (candidate row, column half) ===========================
-        const int q = warp & 3, hc = warp >> 2;                          // TMEM lane quadrant, column half
+        const int q = warp & 3, hc = warp >> 2;                          // TMEM lane quadrant, column group
         const int row = q * 32 + lane;
         const uint32_t tlane = tb + ((uint32_t)(q * 32) << 16);
-        const int c0 = hc * 64;
+        const int c0 = hc * kTcCols;
         constexpr int NB = kMaxN;
         const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
         const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
@@ -260,7 +264,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     for (int j = 0; j < kMaxN; j++) x[j] = j < cfg.n ? a.x0[r0 * cfg.n + j] : 0.f;
                 }
 #pragma unroll 1
-                for (int cc = 0; cc < 64; cc += 16) {
+                for (int cc = 0; cc < kTcCols; cc += 16) {
                     uint32_t v[16], lo[16];
 #pragma unroll
                     for (int j = 0; j < 16; j++) {
@@ -298,10 +302,10 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 const uint32_t dcol = (s & 1) ? kTcColD1 : kTcColD0;
                 const bool was_alive = alive;
                 __syncwarp();
-                // this thread's 64 columns of z_s: four loads in flight, one wait
-                uint32_t r[64];
+                // this thread's kTcCols columns of z_s: all loads in flight, one wait
+                uint32_t r[kTcCols];
 #pragma unroll
-                for (int cc = 0; cc < 64; cc += 16) tmem_ld16(tlane + dcol + c0 + cc, *reinterpret_cast<uint32_t(*)[16]>(&r[cc]));
+                for (int cc = 0; cc < kTcCols; cc += 16) tmem_ld16(tlane + dcol + c0 + cc, *reinterpret_cast<uint32_t(*)[16]>(&r[cc]));
                 uint32_t rp[16];                                         // the physical state sits in columns 0..15
                 if (dump && hc != 0) tmem_ld16(tlane + dcol, rp);
                 wait_ld();
@@ -318,7 +322,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 }
                 if (s < H) {
 #pragma unroll
-                    for (int cc = 0; cc < 64; cc += 8) {
+                    for (int cc = 0; cc < kTcCols; cc += 8) {
                         uint32_t lo[8];
 #pragma unroll
                         for (int j = 0; j < 8; j++) lo[j] = tf32_lo(__uint_as_float(r[cc + j]));
@@ -327,7 +331,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 }
                 if (dump && li < ncand) {                                // a9: traj[(k*J + row)*Ncand + i], k = s-1
 #pragma unroll
-                    for (int j = 0; j < 64; j++) {
+                    for (int j = 0; j < kTcCols; j++) {
                         const int ji = c0 + j;
                         const int orow = ji < cfg.n ? (int)cfg.perm[ji < kMaxN ? ji : 0] : ji;
                         if (orow < J)
@@ -342,7 +346,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
             }
             if (dump && li < ncand) {                                    // states after the tile stopped: NaN
                 for (int k = s - 1; k < H; k++)
-                    for (int j = 0; j < 64; j++) {
+                    for (int j = 0; j < kTcCols; j++) {
                         const int ji = c0 + j;
                         const int orow = ji < cfg.n ? (int)cfg.perm[ji < kMaxN ? ji : 0] : ji;
                         if (orow < J) a.traj[((long long)k * J + orow) * ncand + li] = qnan;
