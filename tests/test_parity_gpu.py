@@ -507,3 +507,36 @@ def test_affine_flag_ignored_with_noise_or_relift(mp):
     assert mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE).info()["variant"] == 1
     w = W.make("C2", N=2000); w.model_kind = 1
     assert mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE).info()["variant"] == 5
+
+
+# ------------------------------------------------------------------ d = 128: both kernels stay covered ------------------
+def test_fp32_tile_kernel_d128_parity(mp):
+    """MPMI_VARIANT_NO_TENSOR keeps the FP32 SIMT warp-tile kernel reachable at d = 128: T1 / T2 and the same winner
+    as the 3xTF32 tcgen05 kernel (the default there)."""
+    w = W.make("C5", N=900)
+    o = _oracle(w)
+    simt = mp.Context(w, variant=mp.mpmi.VARIANT_NO_TENSOR)
+    tens = mp.Context(w)
+    assert simt.info()["variant"] == 2 and tens.info()["variant"] == 4
+    rng = np.random.default_rng(3)
+    U = rng.uniform(w.u_lo, w.u_hi, (w.N, w.m)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, 1)
+    r_steps, r_marg, r_traj = o.rollout_batch(U, x0s, want_traj=True)
+    worst = {}
+    for tag, ctx in (("simt", simt), ("tensor", tens)):
+        traj = torch.full((w.H, w.d, w.N), 7.0, dtype=torch.float32, device="cuda")
+        steps = torch.empty(w.N, dtype=torch.int32, device="cuda")
+        dU, dX = _dev(U), _dev(x0s)
+        ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), 1, w.N, w.H, mp.DUMP_LIFTED, traj.data_ptr(), steps.data_ptr(), 0)
+        torch.cuda.synchronize()
+        g_steps = steps.cpu().numpy(); g_traj = traj.cpu().numpy()
+        bad, _ = check_flags(g_steps, r_steps, r_marg, w.H)
+        assert len(bad) == 0
+        worst[tag] = max(traj_rel_err(g_traj[:, :, i], r_traj[i], min(r_steps[i] + 1, g_steps[i] + 1, w.H)) for i in range(w.N))
+    assert worst["simt"] <= 1e-5 and worst["tensor"] <= TRAJ_RTOL, worst
+    x0s, uus, ticks = W.tick_inputs(w, 6)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        a = simt.step_sync(x0, uu, int(t)).as_dict(w.m); b = tens.step_sync(x0, uu, int(t)).as_dict(w.m)
+        ref = o.step(x0, uu, int(t), detail=True)
+        if (ref["margin_all"] > MARGIN).all():
+            assert (a["index"], a["safe"], a["steps"], a["n_safe"]) == (b["index"], b["safe"], b["steps"], b["n_safe"])
