@@ -103,7 +103,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
 KernFn mpmi_pick_relift(int n, int mode);
 KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
-KernFn mpmi_pick_tc_tick(int *smem, int *threads); KernFn mpmi_pick_tc_batch(int *smem, int *threads);
+KernFn mpmi_pick_tc_tick(int *smem, int *threads, int noise); KernFn mpmi_pick_tc_batch(int *smem, int *threads, int noise);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
 KernFn pick_reg(int D, int M, int P, int mode, bool noise) {
@@ -440,8 +440,8 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     }
 
     // ---- kernel choice ------------------------------------------------------------------------------
-    // prediction noise (Alg. 2 l.5) is built into the register and warp-tile kernels; the latency and tensor-core
-    // kernels do not carry it, so sigma != 0 routes around them
+    // prediction noise (Alg. 2 l.5) is built into the register, warp-tile, tensor-core (n <= 8) and re-lift kernels;
+    // the latency kernel does not carry it, so sigma != 0 routes around it
     const bool noise = cfg->noise_sigma != 0.f;
     dc.noise_sigma = cfg->noise_sigma; dc.model = cfg->model;
     if (cfg->model == MPMI_MODEL_RELIFT) {
@@ -478,13 +478,13 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     } else {
         // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)
         // unless the caller asks for the FP32 SIMT tile kernel; d = 64 stays on the SIMT tile kernel
-        const bool tensor = D == 128 && !noise && !(cfg->variant & MPMI_VARIANT_NO_TENSOR);
+        const bool tensor = D == 128 && (!noise || n <= 8) && !(cfg->variant & MPMI_VARIANT_NO_TENSOR);   // its noise block holds 8 dims
         c->P = 1;
         if (tensor) {
             c->variant = 4;
             int threads = 0;
-            c->k_tick = mpmi_pick_tc_tick(&c->smem, &threads);
-            c->k_batch = mpmi_pick_tc_batch(&c->smem, &threads);
+            c->k_tick = mpmi_pick_tc_tick(&c->smem, &threads, noise);
+            c->k_batch = mpmi_pick_tc_batch(&c->smem, &threads, noise);
             c->block = threads; c->cand_per_block = 128;
         } else {
             c->variant = 2;

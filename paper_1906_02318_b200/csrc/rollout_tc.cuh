@@ -35,7 +35,8 @@
 namespace mpmi {
 
 constexpr int kTcD = 128;                         // padded lifted dim
-constexpr int kTcKD = 136;                        // contraction length: 128 state + 8 input columns (m <= 4, zero padded)
+constexpr int kTcKD = 144;                        // contraction length: 128 state + 8 input columns (m <= 4, zero padded)
+                                                  // + 8 noise columns (n <= 8; used by the NOISE instantiation only)
 constexpr int kTcTile = 128;                      // candidates per tile = TMEM lanes
 #ifndef MPMI_TC_STATE_WARPS
 #define MPMI_TC_STATE_WARPS 8
@@ -47,7 +48,7 @@ constexpr int kTcLBO = 128;                       // bytes between 16-byte K chu
 constexpr int kTcSBO = (kTcKD / 4) * 128;         // bytes between 8-row groups
 constexpr int kTcImg = (kTcD / 8) * kTcSBO;       // bytes of one B-operand image (69,632)
 constexpr int kTcSmemBytes = 2 * kTcImg;
-constexpr uint32_t kTcColD0 = 0, kTcColD1 = 128, kTcColAlo = 256, kTcColUhi = 384, kTcColUlo = 392;
+constexpr uint32_t kTcColD0 = 0, kTcColD1 = 128, kTcColAlo = 256, kTcColUhi = 384, kTcColUlo = 392, kTcColNhi = 400, kTcColNlo = 408;
 
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 // x_lo = x - x_hi (exact) has up to 13 significant bits and the tensor core keeps 11 by TRUNCATION, a bias
@@ -105,7 +106,33 @@ struct TcShared {
     float z0[kTcD];
 };
 
-template <int MODE>
+// sigma * eps of Algorithm 2 l.5 for the tensor-core kernel: the state lives in the accumulator, so the
+// noise enters the contraction as 8 extra A columns [sigma eps_hi | sigma eps_lo] against the selector rows of the K_hi
+// image (1.0 at (r = j, c = 136 + j): exact in TF32, its lo part is 0): z'_j += sigma eps_j through two more MMAs per step.
+__device__ __forceinline__ void tc_noise_store(const DevCfg &cfg, long long gi, int k, unsigned long long tick, uint32_t tlane) {
+    float g[8];                                                  // eps of the ORIGINAL dims 0..7
+#pragma unroll
+    for (int q = 0; q < 2; q++) {
+        float g4[4] = {0.f, 0.f, 0.f, 0.f};
+        if (4 * q < cfg.n) noise4(cfg, gi, k, q, tick, g4);
+#pragma unroll
+        for (int e = 0; e < 4; e++) g[4 * q + e] = g4[e];
+    }
+    uint32_t nh[8], nl[8];
+#pragma unroll
+    for (int j = 0; j < 8; j++) {                                // internal dim j = original dim perm[j]
+        float e = 0.f;
+#pragma unroll
+        for (int p = 0; p < 8; p++) e = ((int)cfg.perm[j] == p) ? g[p] : e;
+        const float v = j < cfg.n ? __fmul_rn(cfg.noise_sigma, e) : 0.f;
+        nh[j] = __float_as_uint(v);
+        nl[j] = tf32_lo(v);
+    }
+    tc::tmem_st8(tlane + kTcColNhi, nh);
+    tc::tmem_st8(tlane + kTcColNlo, nl);
+}
+
+template <int MODE, bool NOISE = false>
 __global__ void __launch_bounds__(kTcThreads, 1)
 rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     using namespace tc;
@@ -124,7 +151,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     // ---- one-off: B-operand images [K | B | 0] split into hi / lo, TMEM, barriers, shared lift
     for (int e = tid; e < kTcD * kTcKD; e += kTcThreads) {
         const int r = e % kTcD, c = e / kTcD;                        // K[r][c] = KTa[c][r]; rows D.. are B's columns
-        const float v = c < kTcD + cfg.m ? cfg.KTa[c * kTcD + r] : 0.f;
+        const float v = c < kTcD + cfg.m ? cfg.KTa[c * kTcD + r] : (c >= 136 && r == c - 136) ? 1.f : 0.f;   // [K | B | 0 | noise selector]
         const float hi = tf32_hi(v);
         const int off = (r >> 3) * kTcSBO + (c >> 2) * kTcLBO + (r & 7) * 16 + (c & 3) * 4;
         *reinterpret_cast<float *>(smem_img + off) = hi;
@@ -210,9 +237,11 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
 #pragma unroll
                     for (int kk = 0; kk < 17; kk++)                        // Z_lo * K_hi
                         mma_tf32_ts(dnxt, kk < 16 ? tb + kTcColAlo + 8 * kk : tb + kTcColUlo, dhi + kk * kstep, idesc, true);
+                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNlo, dhi + 17 * kstep, idesc, true);     // (sigma eps)_lo through the selector
 #pragma unroll
                     for (int kk = 0; kk < 17; kk++)                        // Z_hi * K_hi
                         mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColUhi, dhi + kk * kstep, idesc, true);
+                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + 17 * kstep, idesc, true);     // (sigma eps)_hi
                     mma_commit(bar_full);
                     TCT(ti_23);
                 }
@@ -288,6 +317,8 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     const bool any = __any_sync(0xffffffffu, alive);
                     if (lane == 0) sh.warp_alive[q] = any ? 1u : 0u;
                 }
+                if (NOISE && hc == kTcStateWarps / 4 - 1)          // the last column group draws the noise of step 0
+                    tc_noise_store(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, 0, tick, tlane);
             }
             wait_st();
             fence_before_sync();
@@ -328,6 +359,8 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                         for (int j = 0; j < 8; j++) lo[j] = tf32_lo(__uint_as_float(r[cc + j]));
                         tmem_st8(tlane + kTcColAlo + c0 + cc, lo);
                     }
+                    if (NOISE && hc == kTcStateWarps / 4 - 1)      // noise of MMA step s (it produces z_{s+1})
+                        tc_noise_store(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, s, tick, tlane);
                 }
                 if (dump && li < ncand) {                                // a9: traj[(k*J + row)*Ncand + i], k = s-1
 #pragma unroll
