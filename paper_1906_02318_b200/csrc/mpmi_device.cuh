@@ -117,6 +117,8 @@ __device__ __forceinline__ void noise4(const DevCfg &cfg, long long gi, int k, i
                   cfg.seed_lo, cfg.seed_hi ^ 0x6E6F6973u, w);
 #pragma unroll
     for (int h = 0; h < 2; h++) {
+        g[2 * h] = 0.f; g[2 * h + 1] = 0.f;
+        if (4 * q + 2 * h >= cfg.n) continue;                                              // dims beyond n: no transform (uniform)
         const float u1 = __fmaf_rn(__uint2float_rn(w[2 * h] >> 8), 0x1p-24f, 0x1p-24f);   // ((w >> 8) + 1) 2^-24, exact
         const float u2 = __uint2float_rn(w[2 * h + 1] >> 8) * 0x1p-23f;                    // 2 u2: angle in units of pi
         const float r = sqrtf(-2.0f * logf(u1));

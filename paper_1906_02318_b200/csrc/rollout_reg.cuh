@@ -180,10 +180,8 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
                 }
 #pragma unroll
                 for (int j = 0; j < NB; j++) {
-                    if (j < cfg.n) {                           // internal dim j = original dim perm[j]
-                        float e = 0.f;
-#pragma unroll
-                        for (int p = 0; p < NB; p++) e = ((int)cfg.perm[j] == p) ? g[p] : e;
+                    if (j < cfg.n) {                           // internal dim j = original dim perm[j] (warp-uniform index)
+                        const float e = g[cfg.perm[j]];
                         if (s & 1) z[s >> 1][j].y = __fmaf_rn(cfg.noise_sigma, e, z[s >> 1][j].y);
                         else       z[s >> 1][j].x = __fmaf_rn(cfg.noise_sigma, e, z[s >> 1][j].x);
                     }

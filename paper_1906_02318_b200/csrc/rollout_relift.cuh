@@ -168,10 +168,7 @@ rollout_relift_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant_
 #pragma unroll
             for (int j = 0; j < NP; j++) {
                 if (j < n) {
-                    float e = 0.f;
-#pragma unroll
-                    for (int p = 0; p < NP; p++) e = ((int)cfg.perm[j] == p) ? g[p] : e;
-                    x[j] = __fmaf_rn(cfg.noise_sigma, e, x[j]);
+                    x[j] = __fmaf_rn(cfg.noise_sigma, g[cfg.perm[j] < NP ? cfg.perm[j] : 0], x[j]);
                 }
             }
         }

@@ -121,10 +121,7 @@ __device__ __forceinline__ void tc_noise_store(const DevCfg &cfg, long long gi, 
     uint32_t nh[8], nl[8];
 #pragma unroll
     for (int j = 0; j < 8; j++) {                                // internal dim j = original dim perm[j]
-        float e = 0.f;
-#pragma unroll
-        for (int p = 0; p < 8; p++) e = ((int)cfg.perm[j] == p) ? g[p] : e;
-        const float v = j < cfg.n ? __fmul_rn(cfg.noise_sigma, e) : 0.f;
+        const float v = j < cfg.n ? __fmul_rn(cfg.noise_sigma, g[cfg.perm[j] & 7]) : 0.f;
         nh[j] = __float_as_uint(v);
         nl[j] = tf32_lo(v);
     }
