@@ -319,6 +319,13 @@ __device__ __forceinline__ void mul2_bcast(float2 &acc, float k, const float2 &z
     asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
 }
 
+// NaN-propagating minimum (min.NaN.f32): the safe test as one tree instead of a chain of predicate ANDs
+__device__ __forceinline__ float min_nan(float a, float b) {
+    float d;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+    return d;
+}
+
 __device__ __forceinline__ float4 lds128(unsigned addr) {
     // volatile: keeps the compiler from hoisting the (loop-invariant) model loads out of the
     // horizon loop, which would spill ~D*D registers

@@ -60,11 +60,6 @@ __device__ __forceinline__ uint32_t tf32_lo(float x) { return __float_as_uint(x 
 // the 2*nbox-long chain of dependent predicate ANDs (~13 cycles per link), which sits on the per-step critical
 // path here: lo < x < hi  <=>  min(x - lo, hi - x) > 0 (the sign of an fp32 difference is exact); the minimum
 // over all tested dims is a NaN-propagating tree (min.NaN), and NaN fails the final comparison.
-__device__ __forceinline__ float min_nan(float a, float b) {
-    float d;
-    asm("min.NaN.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
-    return d;
-}
 template <int NB, int J0, int J1>
 __device__ __forceinline__ float box_slack(const DevCfg &cfg, const float (&x)[NB]) {
     if constexpr (J1 - J0 == 1) {
