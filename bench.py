@@ -171,6 +171,56 @@ def run_dump(args, ctx, w, x0s, ticks, stream, info):
         "executed_sample_steps": n_exec, "gpu_launches": K_}))
 
 
+def run_sweep(args, w_full, local):
+    """Scale sweep (BASELINE.json configs[3]): the same model at N = 2^14 .. 2^20 candidates, device-timed tick,
+    host p50 / p99 of mpmi_step_sync, executed sample-steps/s and the FP32 fraction at each N."""
+    import torch
+    import workloads as W
+    import paper_1906_02318_b200 as mp
+    stream = torch.cuda.current_stream().cuda_stream
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    K_, W_ = args.steps, args.warmup
+    rows = []
+    variant = (mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0)
+    for lg in range(14, 21):
+        w = W.make(args.workload, N=1 << lg)
+        w.noise_sigma = args.noise; w.model_kind = 1 if args.relift else 0
+        x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
+        ctx = mp.Context(w, device=local, variant=variant)
+        dX0 = torch.as_tensor(x0s).cuda().contiguous(); dUU = torch.as_tensor(uus).cuda().contiguous()
+        dRes = torch.zeros((W_ + K_, 56), dtype=torch.uint8, device="cuda")
+        for t in range(W_):
+            ctx.step_device(dX0[t].data_ptr(), dUU[t].data_ptr(), int(ticks[t]), stream, dRes[t].data_ptr())
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K_)]
+        torch.cuda.synchronize()
+        for i in range(K_):
+            flush.fill_(i & 0xFF)
+            ev[i][0].record()
+            ctx.step_device(dX0[W_ + i].data_ptr(), dUU[W_ + i].data_ptr(), int(ticks[W_ + i]), stream, dRes[W_ + i].data_ptr())
+            ev[i][1].record()
+        torch.cuda.synchronize()
+        ms = np.array([a.elapsed_time(b) for a, b in ev])
+        res = np.frombuffer(dRes.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)
+        n_exec = int(res["n_exec"][W_:].sum())
+        wall = []
+        for t in range(W_, W_ + K_):
+            t0 = time.perf_counter()
+            ctx.step_sync(np.ascontiguousarray(x0s[t]), np.ascontiguousarray(uus[t]), int(ticks[t]), stream)
+            wall.append(time.perf_counter() - t0)
+        p50, p99 = _percentiles(wall)
+        info = ctx.info()
+        flop = _flop_per_sample_step(w) if info["variant"] != 6 else 2.0 * w.n * w.m
+        rows.append({"N": 1 << lg, "gpu_ms": float(ms.mean()), "host_p50_us": 1e6 * p50, "host_p99_us": 1e6 * p99,
+                     "sample_steps_per_s": n_exec / (ms.sum() * 1e-3), "nominal_sample_steps_per_s": float(w.N + 1) * w.H * K_ / (ms.sum() * 1e-3),
+                     "fp32_frac": n_exec * flop / (ms.sum() * 1e-3) / 1e12 / FP32_PEAK_TFLOPS, "variant": info["variant"]})
+        ctx.close()
+    print(json.dumps({"metric": "rollout sample-steps/s (scale sweep)", "unit": "sample-steps/s", "n_gpus": 1, "steps": K_, "warmup": W_,
+                      "value": rows[-1]["sample_steps_per_s"], "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"{args.workload} scale sweep: n={w_full.n} m={w_full.m} d={w_full.d} H={w_full.H}, N = 2^14 .. 2^20 (+1 user slot)",
+                                 "l2": "256 MB buffer written between timed iterations"},
+                      "sweep": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -186,6 +236,8 @@ def main():
     ap.add_argument("--noise", type=float, default=0.0,
                     help="std of the additive prediction noise of Alg. 2 l.5 (PAPER.md:150); 0 = the noise-free configs of BASELINE.json")
     ap.add_argument("--relift", action="store_true", help="re-lift model x' = C(K Psi(x) + B u) instead of the linear lifted model")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE.json configs[3]: N = 2^14 .. 2^20 on the chosen workload, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
                     help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
     ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
@@ -230,6 +282,8 @@ def main():
     stream = torch.cuda.current_stream().cuda_stream
     if args.dump:
         return run_dump(args, ctx, w, x0s, ticks, stream, info)
+    if args.sweep:
+        return run_sweep(args, w, local)
 
     dX0 = torch.as_tensor(x0s).cuda().contiguous()
     dUU = torch.as_tensor(uus).cuda().contiguous()
