@@ -22,8 +22,8 @@ using namespace mpmi;
 template <int M>
 static KernFn pick_p(int P) {
     constexpr int PW = 32 / MPMI_D;                 // wide packing: 2*PW candidates per thread
-    if (P == 1) return rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE, (MPMI_NOISE != 0)>;
-    if (P == PW) return rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE, (MPMI_NOISE != 0)>;
+    if (P == 1) return reinterpret_cast<KernFn>(rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE, (MPMI_NOISE != 0)>);
+    if (P == PW) return reinterpret_cast<KernFn>(rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE, (MPMI_NOISE != 0)>);
     return nullptr;
 }
 KernFn FN2(MPMI_D)(int M, int P) {

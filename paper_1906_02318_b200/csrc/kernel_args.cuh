@@ -33,6 +33,14 @@ struct KArgs {
     uint8_t *safe;
 };
 
+// The augmented transposed model of the register kernel (D <= 32), passed BY VALUE as a third kernel parameter: kernel
+// parameters live in constant bank 0, so K[r][c] reaches FFMA2 as a uniform-register operand (LDCU on the uniform
+// datapath) instead of through the LSU.  Measured: the same FFMA2 step loop runs at 96 % of the FP32 peak with the
+// model in the constant bank against 88-90 % with warp-uniform LDS.128 (the LSU was the bound).
+struct KModel {
+    float v[(32 + kMaxM) * 32];               // KTa[c * D + r], c < D + m, r < D
+};
+
 enum { MODE_TICK = 0, MODE_BATCH = 1 };
 
 constexpr int kTileNC = 256;                      // candidates per CTA pass of the warp-tile kernel

@@ -21,6 +21,7 @@ using namespace mpmi;
 
 struct mpmi_ctx {
     DevCfg dc;
+    KModel km{};                                      // by-value model parameter of the register kernels (D <= 32)
     int device = 0, sm_count = 0;
     int variant = 0, P = 1, smem = 0, regs = 0;
     int block = 128, cand_per_block = 0;              // launch geometry of the tick kernel
@@ -155,7 +156,7 @@ void launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0,
         if (blocks > c->sm_count) blocks = c->sm_count;
         a.st = c->d_state; a.work = &c->d_state->work;
     }
-    void *args[2] = {(void *)&c->dc, (void *)&a};
+    void *args[3] = {(void *)&c->dc, (void *)&a, (void *)&c->km};   // the register kernels take the model as a third parameter
     cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)smem, s);
 }
 void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
@@ -196,7 +197,7 @@ unsigned grid_for(const mpmi_ctx *c, long long ncand) {
 
 void tick_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
-    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga; args[2] = (void *)&c->km;
     p->func = (void *)c->k_tick; p->gridDim = dim3(c->tick_grid); p->blockDim = dim3((unsigned)c->block);
     p->sharedMemBytes = (unsigned)c->smem; p->kernelParams = args;
 }
@@ -218,7 +219,7 @@ int build_graph(mpmi_ctx *c) {
     if (c->variant == 2 || c->variant == 4) c->ga.work = &c->d_state->work;
     c->tick_grid = grid_for(c, c->dc.shard_count);
     CU(c, cudaGraphCreate(&c->graph, 0));
-    cudaKernelNodeParams p; void *args[2];
+    cudaKernelNodeParams p; void *args[3];
     cudaGraphNode_t dep = nullptr;
     if (c->binning) {
         c->gb = c->bin;
@@ -405,6 +406,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         for (int f = 0; f < d; f++) std::memcpy(&terms[4 * f], &L.terms[4 * po(f)], 4);
 
 #define CUC(call) do { rc = [&]() -> int { CU(c, call); return MPMI_OK; }(); if (rc != MPMI_OK) return bail(rc); } while (0)
+    if (D <= 32) std::memcpy(c->km.v, KTa.data(), KTa.size() * sizeof(float));
     CUC(cudaMalloc(&c->d_KTa, KTa.size() * sizeof(float)));
     CUC(cudaMemcpy(c->d_KTa, KTa.data(), KTa.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUC(cudaMalloc(&c->d_terms, terms.size()));
@@ -581,7 +583,7 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     c->ga.tick_val = tick;
     if (++c->seq == 0) c->seq = 1;
     c->ga.seq = c->seq;
-    cudaKernelNodeParams p; void *args[2];
+    cudaKernelNodeParams p; void *args[3];
     if (c->binning) {
         c->gb.tick_val = tick;
         bin_node_params(c, false, &p, args);

@@ -2,9 +2,10 @@
 //
 // Each thread owns 2P candidates; candidate pair p is packed into the two halves of float2
 // registers so that one FFMA2 (Blackwell packed fp32 FMA, fma.rn.f32x2) advances one row of two
-// candidates: a[p][r] += K[r][c] * z[p][c], the K value broadcast to both halves.  The model is
-// staged once per CTA in shared memory as the augmented transpose KTa[c][r] (c < D: K[r][c];
-// c >= D: B[r][c-D]) and read with warp-uniform LDS.128 (conflict-free broadcast); the candidate's
+// candidates: a[p][r] += K[r][c] * z[p][c], the K value broadcast to both halves.  The model, as the
+// augmented transpose KTa[c][r] (c < D: K[r][c]; c >= D: B[r][c-D]), is a by-value kernel parameter:
+// it sits in the constant bank and enters FFMA2 as a uniform-register operand (kernel_args.cuh:
+// KModel), so the horizon loop issues no load/store-unit instruction at all; the candidate's
 // input u is appended to z as "state" D..D+M-1, so one step executes exactly D*(D+M) fp32 FMAs per
 // candidate -- the algorithmic count of z' = K z + B u.
 // The safe set is tested after every step; a warp leaves the horizon loop when none
@@ -48,16 +49,13 @@ constexpr int reg_min_blocks() { return (D * P >= 32) ? 3 : 4; }
 
 template <int D, int M, int P, int MODE, bool NOISE = false>
 __global__ void __launch_bounds__(kRegBlock, reg_min_blocks<D, P>())
-rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
+rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a, const __grid_constant__ KModel km) {
     constexpr int S = 2 * P;                 // candidates per thread
     constexpr int NB = D < kMaxN ? D : kMaxN;
-    __shared__ __align__(16) float sK[(D + M) * D];
     __shared__ float sz0[D];
     __shared__ float sstage[MODE == MODE_BATCH ? D * kRegBlock : 1];
 
     const int tid = threadIdx.x, bdim = blockDim.x;
-    for (int i = tid; i < (D + M) * D / 4; i += bdim)
-        reinterpret_cast<float4 *>(sK)[i] = reinterpret_cast<const float4 *>(cfg.KTa)[i];
     const unsigned long long tick = a.tick_val;
     const float *x0p = a.inline_inputs ? a.x0_val : a.x0;
     const float *uup = a.inline_inputs ? a.u_val : a.u_user;
@@ -75,7 +73,6 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         for (int f = tid; f < D; f += bdim) sz0[f] = lift_feature(cfg, f, x0p);
     }
     __syncthreads();
-    const unsigned sbase = (unsigned)__cvta_generic_to_shared(sK);
 
     // ---- a1 + a2: candidates of this thread ------------------------------------------------------
     float2 z[P][D + M];
@@ -146,7 +143,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         for (int c = 0; c < D + M; c++) {
 #pragma unroll
             for (int r = 0; r < D; r += 4) {
-                const float4 kv = lds128(sbase + (c * D + r) * 4);
+                const float4 kv = make_float4(km.v[c * D + r], km.v[c * D + r + 1], km.v[c * D + r + 2], km.v[c * D + r + 3]);
 #pragma unroll
                 for (int p = 0; p < P; p++) {
                     const float2 zc = z[p][c];
