@@ -20,18 +20,30 @@ using namespace mpmi;
 #define FN2(D) FN(D)
 
 template <int M>
-static KernFn pick_p(int P) {
+static KernFn pick_p(int P, int kconst) {
     constexpr int PW = 32 / MPMI_D;                 // wide packing: 2*PW candidates per thread
-    if (P == 1) return reinterpret_cast<KernFn>(rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE, (MPMI_NOISE != 0)>);
-    if (P == PW) return reinterpret_cast<KernFn>(rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE, (MPMI_NOISE != 0)>);
+    if (!kconst) {                               // shared-memory model (small grids, or no free constant slot)
+        if (P == 1) return rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE, (MPMI_NOISE != 0), false>;
+        if (P == PW) return rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE, (MPMI_NOISE != 0), false>;
+    }
+    if (P == 1) return rollout_reg_kernel<MPMI_D, M, 1, MPMI_MODE, (MPMI_NOISE != 0), true>;
+    if (P == PW) return rollout_reg_kernel<MPMI_D, M, PW, MPMI_MODE, (MPMI_NOISE != 0), true>;
     return nullptr;
 }
-KernFn FN2(MPMI_D)(int M, int P) {
+KernFn FN2(MPMI_D)(int M, int P, int kconst) {
     switch (M) {
-        case 1: return pick_p<1>(P);
-        case 2: return pick_p<2>(P);
-        case 3: return pick_p<3>(P);
-        case 4: return pick_p<4>(P);
+        case 1: return pick_p<1>(P, kconst);
+        case 2: return pick_p<2>(P, kconst);
+        case 3: return pick_p<3>(P, kconst);
+        case 4: return pick_p<4>(P, kconst);
     }
     return nullptr;
+}
+
+// fills constant-memory slot `slot` of THIS translation unit with the context's augmented transposed model
+#define SETFN3(a, b) a##b
+#define SETFN2(a, b) SETFN3(a, b)
+int SETFN2(FN2(MPMI_D), _setmodel)(int slot, const float *kta, int nfloats) {
+    if (slot < 0 || slot >= kModelSlots || nfloats > kModelFloats) return (int)cudaErrorInvalidValue;
+    return (int)cudaMemcpyToSymbol(c_model, kta, sizeof(float) * nfloats, sizeof(float) * kModelFloats * slot, cudaMemcpyHostToDevice);
 }

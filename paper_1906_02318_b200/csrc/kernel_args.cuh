@@ -15,6 +15,7 @@ struct KArgs {
     float x0_val[kMaxN];
     float u_val[kMaxM];
     int inline_inputs;                    // 1: read x0_val / u_val instead of x0 / u_user
+    int kslot;                            // constant-memory slot of this context's model (register kernels)
     unsigned seq;                         // written last into out->reserved (host polls it on mapped memory)
     TickState *st;
     mpmi_result *out;
@@ -33,13 +34,13 @@ struct KArgs {
     uint8_t *safe;
 };
 
-// The augmented transposed model of the register kernel (D <= 32), passed BY VALUE as a third kernel parameter: kernel
-// parameters live in constant bank 0, so K[r][c] reaches FFMA2 as a uniform-register operand (LDCU on the uniform
-// datapath) instead of through the LSU.  Measured: the same FFMA2 step loop runs at 96 % of the FP32 peak with the
-// model in the constant bank against 88-90 % with warp-uniform LDS.128 (the LSU was the bound).
-struct KModel {
-    float v[(32 + kMaxM) * 32];               // KTa[c * D + r], c < D + m, r < D
-};
+// The augmented transposed model of the register kernels (D <= 32) lives in __constant__ memory, one slot per context
+// (rollout_reg.cuh: c_model): K[r][c] then reaches FFMA2 as a uniform-register operand (LDCU on the uniform datapath)
+// instead of through the LSU.  Measured: the same FFMA2 step loop runs at 96 % of the FP32 peak with the model in the
+// constant bank against 88-90 % with warp-uniform LDS.128 (the LSU was the bound).  (A 4.6 KB by-value kernel parameter
+// gives the same SASS but costs 160 s of cicc time per instantiation.)
+constexpr int kModelSlots = 8;
+constexpr int kModelFloats = (32 + kMaxM) * 32;
 
 enum { MODE_TICK = 0, MODE_BATCH = 1 };
 

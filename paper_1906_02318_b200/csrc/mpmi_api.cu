@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -21,7 +22,7 @@ using namespace mpmi;
 
 struct mpmi_ctx {
     DevCfg dc;
-    KModel km{};                                      // by-value model parameter of the register kernels (D <= 32)
+    int kslot = -1;                                   // constant-memory slot of the model (register kernels), -1 = none
     int device = 0, sm_count = 0;
     int variant = 0, P = 1, smem = 0, regs = 0;
     int block = 128, cand_per_block = 0;              // launch geometry of the tick kernel
@@ -99,8 +100,10 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 }
 
 // kernel tables live in inst_reg.cu / inst_tile.cu, one translation unit per (D, MODE)
-#define MPMI_DECL_REG(D) KernFn mpmi_pick_reg_##D##_tick(int M, int P); KernFn mpmi_pick_reg_##D##_batch(int M, int P); \
-                         KernFn mpmi_pick_regn_##D##_tick(int M, int P); KernFn mpmi_pick_regn_##D##_batch(int M, int P);
+#define MPMI_DECL_REG(D) KernFn mpmi_pick_reg_##D##_tick(int M, int P, int kconst); KernFn mpmi_pick_reg_##D##_batch(int M, int P, int kconst); \
+                         KernFn mpmi_pick_regn_##D##_tick(int M, int P, int kconst); KernFn mpmi_pick_regn_##D##_batch(int M, int P, int kconst); \
+                         int mpmi_pick_reg_##D##_tick_setmodel(int, const float *, int); int mpmi_pick_reg_##D##_batch_setmodel(int, const float *, int); \
+                         int mpmi_pick_regn_##D##_tick_setmodel(int, const float *, int); int mpmi_pick_regn_##D##_batch_setmodel(int, const float *, int);
 #define MPMI_DECL_TILE(D) KernFn mpmi_pick_tile_##D##_tick(int M, int *smem); KernFn mpmi_pick_tile_##D##_batch(int M, int *smem); \
                           KernFn mpmi_pick_tilen_##D##_tick(int M, int *smem); KernFn mpmi_pick_tilen_##D##_batch(int M, int *smem);
 }  // namespace
@@ -110,23 +113,46 @@ KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
 KernFn mpmi_pick_tc_tick(int *smem, int *threads, int noise); KernFn mpmi_pick_tc_batch(int *smem, int *threads, int noise);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
-KernFn pick_reg(int D, int M, int P, int mode, bool noise) {
+KernFn pick_reg(int D, int M, int P, int mode, bool noise, int kconst = 1) {
     const bool t = mode == MODE_TICK;
     if (noise) {
         switch (D) {
-            case 8: return t ? mpmi_pick_regn_8_tick(M, P) : mpmi_pick_regn_8_batch(M, P);
-            case 16: return t ? mpmi_pick_regn_16_tick(M, P) : mpmi_pick_regn_16_batch(M, P);
-            case 32: return t ? mpmi_pick_regn_32_tick(M, P) : mpmi_pick_regn_32_batch(M, P);
+            case 8: return t ? mpmi_pick_regn_8_tick(M, P, kconst) : mpmi_pick_regn_8_batch(M, P, kconst);
+            case 16: return t ? mpmi_pick_regn_16_tick(M, P, kconst) : mpmi_pick_regn_16_batch(M, P, kconst);
+            case 32: return t ? mpmi_pick_regn_32_tick(M, P, kconst) : mpmi_pick_regn_32_batch(M, P, kconst);
         }
         return nullptr;
     }
     switch (D) {
-        case 8: return t ? mpmi_pick_reg_8_tick(M, P) : mpmi_pick_reg_8_batch(M, P);
-        case 16: return t ? mpmi_pick_reg_16_tick(M, P) : mpmi_pick_reg_16_batch(M, P);
-        case 32: return t ? mpmi_pick_reg_32_tick(M, P) : mpmi_pick_reg_32_batch(M, P);
+        case 8: return t ? mpmi_pick_reg_8_tick(M, P, kconst) : mpmi_pick_reg_8_batch(M, P, kconst);
+        case 16: return t ? mpmi_pick_reg_16_tick(M, P, kconst) : mpmi_pick_reg_16_batch(M, P, kconst);
+        case 32: return t ? mpmi_pick_reg_32_tick(M, P, kconst) : mpmi_pick_reg_32_batch(M, P, kconst);
     }
     return nullptr;
 }
+// constant-memory model slots of the register kernels: one per live context (kernel_args.cuh: kModelSlots)
+std::mutex g_slot_mu;
+bool g_slot_used[kModelSlots] = {};
+int slot_acquire() {
+    std::lock_guard<std::mutex> lk(g_slot_mu);
+    for (int i = 0; i < kModelSlots; i++) if (!g_slot_used[i]) { g_slot_used[i] = true; return i; }
+    return -1;
+}
+void slot_release(int i) {
+    if (i < 0) return;
+    std::lock_guard<std::mutex> lk(g_slot_mu);
+    g_slot_used[i] = false;
+}
+// the slot is filled in the translation units of the tick and batch kernels this context launches
+int set_model(int D, bool noise, int slot, const float *kta, int nfloats) {
+    int rc = 0;
+#define MPMI_SET(D_) case D_: rc = noise ? (mpmi_pick_regn_##D_##_tick_setmodel(slot, kta, nfloats) | mpmi_pick_regn_##D_##_batch_setmodel(slot, kta, nfloats)) \
+                                          : (mpmi_pick_reg_##D_##_tick_setmodel(slot, kta, nfloats) | mpmi_pick_reg_##D_##_batch_setmodel(slot, kta, nfloats)); break;
+    switch (D) { MPMI_SET(8) MPMI_SET(16) MPMI_SET(32) default: rc = (int)cudaErrorInvalidValue; }
+#undef MPMI_SET
+    return rc;
+}
+
 KernFn pick_lat(int D, int M, int R) {
     return D == 8 ? mpmi_pick_lat_8(M, R) : D == 16 ? mpmi_pick_lat_16(M, R) : D == 32 ? mpmi_pick_lat_32(M, R) : nullptr;
 }
@@ -156,7 +182,8 @@ void launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0,
         if (blocks > c->sm_count) blocks = c->sm_count;
         a.st = c->d_state; a.work = &c->d_state->work;
     }
-    void *args[3] = {(void *)&c->dc, (void *)&a, (void *)&c->km};   // the register kernels take the model as a third parameter
+    a.kslot = c->kslot;
+    void *args[2] = {(void *)&c->dc, (void *)&a};
     cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)smem, s);
 }
 void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
@@ -197,7 +224,7 @@ unsigned grid_for(const mpmi_ctx *c, long long ncand) {
 
 void tick_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
-    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga; args[2] = (void *)&c->km;
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
     p->func = (void *)c->k_tick; p->gridDim = dim3(c->tick_grid); p->blockDim = dim3((unsigned)c->block);
     p->sharedMemBytes = (unsigned)c->smem; p->kernelParams = args;
 }
@@ -215,11 +242,11 @@ void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **
 
 int build_graph(mpmi_ctx *c) {
     c->ga = KArgs{};
-    c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1;
+    c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1; c->ga.kslot = c->kslot;
     if (c->variant == 2 || c->variant == 4) c->ga.work = &c->d_state->work;
     c->tick_grid = grid_for(c, c->dc.shard_count);
     CU(c, cudaGraphCreate(&c->graph, 0));
-    cudaKernelNodeParams p; void *args[3];
+    cudaKernelNodeParams p; void *args[2];
     cudaGraphNode_t dep = nullptr;
     if (c->binning) {
         c->gb = c->bin;
@@ -271,6 +298,7 @@ void mpmi_destroy(mpmi_ctx *c) {
     if (c->graph) cudaGraphDestroy(c->graph);
     cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
     cudaFree(c->d_state);
+    slot_release(c->kslot);
     cudaFree(c->d_affA); cudaFree(c->d_affG);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_res);
@@ -406,7 +434,6 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         for (int f = 0; f < d; f++) std::memcpy(&terms[4 * f], &L.terms[4 * po(f)], 4);
 
 #define CUC(call) do { rc = [&]() -> int { CU(c, call); return MPMI_OK; }(); if (rc != MPMI_OK) return bail(rc); } while (0)
-    if (D <= 32) std::memcpy(c->km.v, KTa.data(), KTa.size() * sizeof(float));
     CUC(cudaMalloc(&c->d_KTa, KTa.size() * sizeof(float)));
     CUC(cudaMemcpy(c->d_KTa, KTa.data(), KTa.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUC(cudaMalloc(&c->d_terms, terms.size()));
@@ -471,9 +498,18 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         c->cand_per_block = 2 * c->P * c->block;
         c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
         c->smem = 0;
-        c->k_tick = pick_reg(D, M, c->P, MODE_TICK, noise);
-        c->k_batch = pick_reg(D, M, c->P, MODE_BATCH, noise);
-        c->k_batch_dump = pick_reg(D, M, 1, MODE_BATCH, noise);
+        // model source: the constant bank (one slot per context) when the grid fills the machine or the model fits the
+        // immediate constant cache, shared memory otherwise (measured crossover at D = 32: ~2^19 candidates); the batch
+        // kernels take the constant bank whenever a slot is free (it frees the LSU for the trajectory stores)
+        c->kslot = slot_acquire();
+        if (c->kslot >= 0 && set_model(D, noise, c->kslot, KTa.data(), (int)KTa.size()) != 0) {
+            slot_release(c->kslot); c->kslot = -1; (void)cudaGetLastError();
+        }
+        const int kconst_tick = (c->kslot >= 0 && ((D + M) * D * 4 <= 2048 || sc >= (1LL << 19))) ? 1 : 0;
+        const int kconst_batch = c->kslot >= 0 ? 1 : 0;
+        c->k_tick = pick_reg(D, M, c->P, MODE_TICK, noise, kconst_tick);
+        c->k_batch = pick_reg(D, M, c->P, MODE_BATCH, noise, kconst_batch);
+        c->k_batch_dump = pick_reg(D, M, 1, MODE_BATCH, noise, kconst_batch);
         // paper-scale candidate sets: 4 lanes per candidate (rollout_lat.cuh) shorten the dependent chain
         const bool lat = !noise && ((cfg->variant & MPMI_VARIANT_LATENCY) || (!(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE)) && sc <= kLatMaxCand));
         if (lat && !c->binning) {
@@ -583,7 +619,7 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     c->ga.tick_val = tick;
     if (++c->seq == 0) c->seq = 1;
     c->ga.seq = c->seq;
-    cudaKernelNodeParams p; void *args[3];
+    cudaKernelNodeParams p; void *args[2];
     if (c->binning) {
         c->gb.tick_val = tick;
         bin_node_params(c, false, &p, args);

@@ -3,9 +3,9 @@
 // Each thread owns 2P candidates; candidate pair p is packed into the two halves of float2
 // registers so that one FFMA2 (Blackwell packed fp32 FMA, fma.rn.f32x2) advances one row of two
 // candidates: a[p][r] += K[r][c] * z[p][c], the K value broadcast to both halves.  The model, as the
-// augmented transpose KTa[c][r] (c < D: K[r][c]; c >= D: B[r][c-D]), is a by-value kernel parameter:
-// it sits in the constant bank and enters FFMA2 as a uniform-register operand (kernel_args.cuh:
-// KModel), so the horizon loop issues no load/store-unit instruction at all; the candidate's
+// augmented transpose KTa[c][r] (c < D: K[r][c]; c >= D: B[r][c-D]), sits in __constant__ memory and
+// enters FFMA2 as a uniform-register operand (kernel_args.cuh), so the horizon loop issues no
+// load/store-unit instruction at all (shared memory + LDS.128 remains as the KC = false variant); the candidate's
 // input u is appended to z as "state" D..D+M-1, so one step executes exactly D*(D+M) fp32 FMAs per
 // candidate -- the algorithmic count of z' = K z + B u.
 // The safe set is tested after every step; a warp leaves the horizon loop when none
@@ -44,14 +44,27 @@ __device__ __forceinline__ bool safe_check(const DevCfg &cfg, const float (&x)[N
     return ok;
 }
 
+// model slots in constant memory (one copy of this array per translation unit: no relocatable device code; the
+// host fills the slot of a context in every translation unit whose kernels it launches, see inst_reg.cu)
+static __constant__ float4 c_model[kModelSlots][kModelFloats / 4];
+
 template <int D, int P>
 constexpr int reg_min_blocks() { return (D * P >= 32) ? 3 : 4; }
 
-template <int D, int M, int P, int MODE, bool NOISE = false>
+// KC = true: model values from the constant bank (slot a.kslot of c_model), the choice for grids that fill the machine;
+// KC = false: staged in shared memory and read with warp-uniform LDS.128 -- better when an SM holds only one or two
+// warps, which cannot hide the constant-cache misses of a 4.3 KB model (measured crossover: ~2^19 candidates at D = 32).
+template <int D, int M, int P, int MODE, bool NOISE = false, bool KC = true>
 __global__ void __launch_bounds__(kRegBlock, reg_min_blocks<D, P>())
-rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a, const __grid_constant__ KModel km) {
+rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     constexpr int S = 2 * P;                 // candidates per thread
     constexpr int NB = D < kMaxN ? D : kMaxN;
+    __shared__ __align__(16) float sK[KC ? 4 : (D + M) * D];
+    if (!KC) {
+        for (int i = threadIdx.x; i < (D + M) * D / 4; i += blockDim.x)
+            reinterpret_cast<float4 *>(sK)[i] = reinterpret_cast<const float4 *>(cfg.KTa)[i];
+    }
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(sK);
     __shared__ float sz0[D];
     __shared__ float sstage[MODE == MODE_BATCH ? D * kRegBlock : 1];
 
@@ -143,7 +156,8 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         for (int c = 0; c < D + M; c++) {
 #pragma unroll
             for (int r = 0; r < D; r += 4) {
-                const float4 kv = make_float4(km.v[c * D + r], km.v[c * D + r + 1], km.v[c * D + r + 2], km.v[c * D + r + 3]);
+                const float4 kv = KC ? c_model[a.kslot][(c * D + r) / 4]
+                                     : lds128(sbase + (c * D + r) * 4);
 #pragma unroll
                 for (int p = 0; p < P; p++) {
                     const float2 zc = z[p][c];
