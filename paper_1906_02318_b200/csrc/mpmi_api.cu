@@ -490,14 +490,6 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     } else if (D <= 32) {
         c->variant = 1;
         const int Pmax = 32 / D;
-        // enough warps to give every SM sub-partition two warps at the wide packing?  else 2 cand/thread
-        const long long warps_wide = (sc + 2LL * Pmax * 32 - 1) / (2LL * Pmax * 32);
-        c->P = (cfg->variant & MPMI_VARIANT_NARROW) ? 1 : (cfg->variant & MPMI_VARIANT_WIDE) ? Pmax : (warps_wide >= 8LL * c->sm_count ? Pmax : 1);
-        const long long threads = (sc + 2LL * c->P - 1) / (2LL * c->P);
-        c->block = threads >= 128LL * 2 * c->sm_count ? 128 : threads >= 64LL * 2 * c->sm_count ? 64 : 32;
-        c->cand_per_block = 2 * c->P * c->block;
-        c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
-        c->smem = 0;
         // model source: the constant bank (one slot per context) when the grid fills the machine or the model fits the
         // immediate constant cache, shared memory otherwise (measured crossover at D = 32: ~2^19 candidates); the batch
         // kernels take the constant bank whenever a slot is free (it frees the LSU for the trajectory stores)
@@ -507,6 +499,15 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         }
         const int kconst_tick = (c->kslot >= 0 && ((D + M) * D * 4 <= 2048 || sc >= (1LL << 19))) ? 1 : 0;
         const int kconst_batch = c->kslot >= 0 ? 1 : 0;
+        // shared-memory model: enough warps to give every SM sub-partition two warps at the wide packing?  else 2 cand/thread
+        const long long warps_wide = (sc + 2LL * Pmax * 32 - 1) / (2LL * Pmax * 32);
+        c->P = (cfg->variant & MPMI_VARIANT_NARROW) ? 1 : (cfg->variant & MPMI_VARIANT_WIDE) ? Pmax
+               : kconst_tick ? 1 : (warps_wide >= 8LL * c->sm_count ? Pmax : 1);   // constant-bank model: 2 per thread is faster (measured)
+        const long long threads = (sc + 2LL * c->P - 1) / (2LL * c->P);
+        c->block = threads >= 128LL * 2 * c->sm_count ? 128 : threads >= 64LL * 2 * c->sm_count ? 64 : 32;
+        c->cand_per_block = 2 * c->P * c->block;
+        c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
+        c->smem = 0;
         c->k_tick = pick_reg(D, M, c->P, MODE_TICK, noise, kconst_tick);
         c->k_batch = pick_reg(D, M, c->P, MODE_BATCH, noise, kconst_batch);
         c->k_batch_dump = pick_reg(D, M, 1, MODE_BATCH, noise, kconst_batch);
