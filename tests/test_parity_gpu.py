@@ -540,3 +540,22 @@ def test_fp32_tile_kernel_d128_parity(mp):
         ref = o.step(x0, uu, int(t), detail=True)
         if (ref["margin_all"] > MARGIN).all():
             assert (a["index"], a["safe"], a["steps"], a["n_safe"]) == (b["index"], b["safe"], b["steps"], b["n_safe"])
+
+
+def test_constant_slot_exhaustion_falls_back_to_shared_memory(mp):
+    """The register kernels keep the model in one of 8 __constant__ slots per live context; a 9th, 10th ... context must
+    fall back to the shared-memory variant and return identical results (and slots are recycled on close)."""
+    w = W.make("C4", N=1 << 19)
+    x0s, uus, ticks = W.tick_inputs(w, 2)
+    ctxs = [mp.Context(w) for _ in range(11)]
+    ref = [ctxs[0].step_sync(x0, uu, int(t)).as_dict(w.m) for x0, uu, t in zip(x0s, uus, ticks)]
+    for c in ctxs[1:]:
+        for r0, (x0, uu, t) in zip(ref, zip(x0s, uus, ticks)):
+            r = c.step_sync(x0, uu, int(t)).as_dict(w.m)
+            assert (r["index"], r["safe"], r["steps"], r["n_safe"], r["n_exec"], r["key"]) == \
+                   (r0["index"], r0["safe"], r0["steps"], r0["n_safe"], r0["n_exec"], r0["key"])
+    for c in ctxs:
+        c.close()
+    again = mp.Context(w)                                  # a slot is free again
+    r = again.step_sync(x0s[0], uus[0], int(ticks[0])).as_dict(w.m)
+    assert r["key"] == ref[0]["key"]
