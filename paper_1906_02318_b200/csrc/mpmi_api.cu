@@ -80,7 +80,7 @@ __global__ void shard_finalise_kernel(const __grid_constant__ DevCfg cfg, const 
 
 namespace {
 
-constexpr long long kLatMaxCand = 1 << 15;      // <= this many candidates: latency kernel (measured crossover)
+constexpr long long kLatMaxCand = 24576;        // <= this many candidates: latency kernel (measured: 125 vs 155 us at 2^14, 210 vs 164 us at 2^15)
 
 thread_local std::string g_create_err;
 
@@ -456,7 +456,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     {
         const long long send = sb + sc < cfg->N ? sb + sc : cfg->N;
         const long long nsamp = send > sb ? send - sb : 0;
-        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (1 << 15);
+        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (D > 32 ? (1 << 15) : (1 << 17));   // measured at d = 32: the ~25 us of binning pay from 2^17 up
         c->binning = (cfg->variant & MPMI_VARIANT_FORCE_BINNING) ? (cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= 64)
                                                                   : (want && !(cfg->variant & MPMI_VARIANT_NO_BINNING));
         if (c->binning) {
