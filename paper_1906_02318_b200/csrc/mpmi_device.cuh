@@ -319,6 +319,35 @@ __device__ __forceinline__ void mul2_bcast(float2 &acc, float k, const float2 &z
     asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
 }
 
+// ---- a4: isSafe(x) -----------------------------------------------------
+// box limits on internal dims 0..nbox-1 (strict), annulus on internal dims 0,1 (closed); NaN -> unsafe
+template <int NB>
+__device__ __forceinline__ bool safe_check(const DevCfg &cfg, const float (&x)[NB], int nbox) {
+    bool ok = true;
+    if (nbox > 0) {
+#pragma unroll
+        for (int j = 0; j < 2 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+        if (nbox > 2) {
+#pragma unroll
+            for (int j = 2; j < 4 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+            if (nbox > 4) {
+#pragma unroll
+                for (int j = 4; j < 8 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+                if (nbox > 8) {
+#pragma unroll
+                    for (int j = 8; j < 16 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+                }
+            }
+        }
+    }
+    if (cfg.annulus) {
+        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
+        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
+        ok = ok && (r2 >= cfg.rmin2) && (r2 <= cfg.rmax2);
+    }
+    return ok;
+}
+
 // NaN-propagating minimum (min.NaN.f32): the safe test as one tree instead of a chain of predicate ANDs
 __device__ __forceinline__ float min_nan(float a, float b) {
     float d;

@@ -11,7 +11,7 @@
 // so its rounding order differs from rollout_reg_kernel by one reassociation (well inside T1).
 #pragma once
 #include "mpmi_device.cuh"
-#include "rollout_reg.cuh"
+#include "kernel_args.cuh"
 
 namespace mpmi {
 

@@ -16,34 +16,6 @@
 
 namespace mpmi {
 
-// box limits on internal dims 0..nbox-1 (strict), annulus on internal dims 0,1 (closed); NaN -> unsafe
-template <int NB>
-__device__ __forceinline__ bool safe_check(const DevCfg &cfg, const float (&x)[NB], int nbox) {
-    bool ok = true;
-    if (nbox > 0) {
-#pragma unroll
-        for (int j = 0; j < 2 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
-        if (nbox > 2) {
-#pragma unroll
-            for (int j = 2; j < 4 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
-            if (nbox > 4) {
-#pragma unroll
-                for (int j = 4; j < 8 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
-                if (nbox > 8) {
-#pragma unroll
-                    for (int j = 8; j < 16 && j < NB; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
-                }
-            }
-        }
-    }
-    if (cfg.annulus) {
-        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
-        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
-        ok = ok && (r2 >= cfg.rmin2) && (r2 <= cfg.rmax2);
-    }
-    return ok;
-}
-
 // model slots in constant memory (one copy of this array per translation unit: no relocatable device code; the
 // host fills the slot of a context in every translation unit whose kernels it launches, see inst_reg.cu)
 static __constant__ float4 c_model[kModelSlots][kModelFloats / 4];

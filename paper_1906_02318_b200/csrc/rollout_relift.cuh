@@ -14,7 +14,6 @@
 #pragma once
 #include "mpmi_device.cuh"
 #include "kernel_args.cuh"
-#include "rollout_reg.cuh"
 
 namespace mpmi {
 

@@ -29,7 +29,6 @@
 #pragma once
 #include "mpmi_device.cuh"
 #include "kernel_args.cuh"
-#include "rollout_reg.cuh"
 #include "tcgen05.cuh"
 
 namespace mpmi {
@@ -56,7 +55,7 @@ __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__flo
 // to the bit pattern first turns the hardware's truncation into round-half-away (one integer add).
 __device__ __forceinline__ uint32_t tf32_lo(float x) { return __float_as_uint(x - tf32_hi(x)) + 0x1000u; }
 
-// Same decision as safe_check (rollout_reg.cuh) -- box strict, annulus closed, NaN / Inf unsafe -- but without
+// Same decision as safe_check (mpmi_device.cuh) -- box strict, annulus closed, NaN / Inf unsafe -- but without
 // the 2*nbox-long chain of dependent predicate ANDs (~13 cycles per link), which sits on the per-step critical
 // path here: lo < x < hi  <=>  min(x - lo, hi - x) > 0 (the sign of an fp32 difference is exact); the minimum
 // over all tested dims is a NaN-propagating tree (min.NaN), and NaN fails the final comparison.

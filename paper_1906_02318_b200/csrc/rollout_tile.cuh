@@ -14,7 +14,7 @@
 // inside the horizon loop.
 #pragma once
 #include "mpmi_device.cuh"
-#include "rollout_reg.cuh"
+#include "kernel_args.cuh"
 
 namespace mpmi {
 
