@@ -260,9 +260,16 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dist = None
-    if world > 1:
+    # MPMI_BENCH_FORCE_SHARD=1 runs the sharded (multi-GPU) code path on one rank: a real single-rank NCCL group,
+    # shard_step -> all-gather -> shard_finalize, so that the N > 1 path can be exercised on a 1-GPU box
+    sharded = world > 1 or os.environ.get("MPMI_BENCH_FORCE_SHARD") == "1"
+    if sharded:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29531")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     # ---- workload: weak scaling -- every rank owns N_per candidates of a global set of world*N_per
     w1 = W.make(args.workload, N=args.N)
@@ -276,7 +283,7 @@ def main():
     x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
     begin, count = shard_plan(w.N, 1, world, rank)             # the injected u_user (index N) goes to the last rank
-    ctx = mp.Context(w, device=local, shard=(begin, count) if world > 1 else (0, 0),
+    ctx = mp.Context(w, device=local, shard=(begin, count) if sharded else (0, 0),
                      variant=(mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0))
     info = ctx.info()
     stream = torch.cuda.current_stream().cuda_stream
@@ -293,7 +300,7 @@ def main():
 
     def tick_device(t):
         px, pu, pr = dX0[t].data_ptr(), dUU[t].data_ptr(), dRes[t].data_ptr()
-        if world == 1:
+        if not sharded:
             ctx.step_device(px, pu, int(ticks[t]), stream, pr)
         else:                                                  # shard -> 24-byte all-gather -> finalise
             ctx.shard_step(px, pu, int(ticks[t]), stream, dPart.data_ptr())
@@ -332,7 +339,7 @@ def main():
     # ---- e2e: the public host API, host buffers, H2D + D2H inside the timed region (N = 1 only)
     e2e = None
     lat = {}
-    if world == 1:
+    if not sharded:
         r = mp.Result()
         x0c = [np.ascontiguousarray(x) for x in x0s]; uuc = [np.ascontiguousarray(u) for u in uus]
         for t in range(W_):
@@ -370,6 +377,38 @@ def main():
             p50, p99 = _percentiles(wall)
             lat["C2_N10000"] = {"host_p50_us": 1e6 * p50, "host_p99_us": 1e6 * p99, "ticks": len(seq)}
             c2.close()
+
+    if sharded:
+        # e2e at N GPUs: x0 / u_user from pinned host memory every tick, sharded tick, 24-byte exchange, result back to the host
+        try:
+            hx = torch.as_tensor(x0s).contiguous().pin_memory(); hu = torch.as_tensor(uus).contiguous().pin_memory()
+            hres = torch.zeros(56, dtype=torch.uint8).pin_memory()
+            dx = torch.empty(w.n, dtype=torch.float32, device="cuda"); du = torch.empty(w.m, dtype=torch.float32, device="cuda")
+            dres = torch.zeros(56, dtype=torch.uint8, device="cuda")
+            cur = torch.cuda.current_stream()
+
+            def tick_e2e(t):
+                dx.copy_(hx[t], non_blocking=True); du.copy_(hu[t], non_blocking=True)
+                ctx.shard_step(dx.data_ptr(), du.data_ptr(), int(ticks[t]), stream, dPart.data_ptr())
+                parts = gather_partials(dPart, world)
+                ctx.shard_finalize(parts.data_ptr(), world, du.data_ptr(), int(ticks[t]), stream, dres.data_ptr())
+                hres.copy_(dres, non_blocking=True)
+                cur.synchronize()
+                return int(np.frombuffer(hres.numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)[0]["n_exec"])
+
+            for t in range(W_):
+                tick_e2e(t)
+            dist.barrier()
+            t_all = time.perf_counter()
+            e_exec = sum(tick_e2e(t) for t in range(W_, W_ + K_))
+            t_all = time.perf_counter() - t_all
+            tm = torch.tensor([t_all], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+            e2e = {"value": e_exec / float(tm.item()), "unit": "sample-steps/s", "h2d_bytes_per_step": 4 * (w.n + w.m), "d2h_bytes_per_step": 56,
+                   "transport": "per rank: x0, u_user copied from pinned host memory, sharded tick, 24-byte NCCL all-gather, 56-byte result copied back",
+                   "ms_per_step": 1e3 * float(tm.item()) / K_}
+        except Exception as ex:                                  # never lose the bench line over the e2e leg
+            e2e = {"value": None, "unit": "sample-steps/s", "error": repr(ex)[:200]}
 
     # ---- roofline of the dominant (only) kernel: plain FP32 FMA arithmetic
     flop = _flop_per_sample_step(w) if info["variant"] != 6 else 2.0 * w.n * w.m      # affine path: n*m FMAs per sample-step
@@ -434,11 +473,11 @@ def main():
                                + (", re-lift model" if args.relift else "")
                                + (", affine-in-u fast path (NEXT-4: separate metric, 2nm flop per sample-step)" if info["variant"] == 6 else ""),
                    "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
-                   "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if world > 1 else "single GPU",
+                   "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if sharded else "single GPU",
                    "kernel": info},
         "nominal_value": nominal / (total_ms * 1e-3), "executed_fraction": n_exec / nominal,
         "safe_fraction": float(res["n_safe"][W_:].mean() / (w.N + 1)),
-        "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": K_ * (info["launches_per_tick"] + (1 if world > 1 else 0)),
+        "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": K_ * (info["launches_per_tick"] + (1 if sharded else 0)),
         "roofline": roofline, "cpu_baseline": cpu, "latency": lat,
         "paper_context": "paper: >10,000 trajectories per tick at ~100 Hz / ~60 Hz on a GeForce 860M (PAPER.md:12, 266)",
     }
