@@ -26,7 +26,7 @@ rollout_relift_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant_
     constexpr int NB = kMaxN;                                   // safe_check works on 16 internal dims
     __shared__ __align__(16) float sKp[(MPMI_MAX_D + kMaxM) * NP]; // Kp[c][r] = K[r][c] (c < d), B[r][c-d]; rows r < n, else 0
     __shared__ float sval[(1 + 3 * NP) * kRlBlock];             // slot s of thread t at sval[s * kRlBlock + t]
-    __shared__ unsigned sslot[MPMI_MAX_D];                      // MONO: four slot indices per feature, one byte each
+    __shared__ unsigned sslot[MPMI_MAX_D];                      // MONO: up to four 6-bit slot indices per feature + their count
 
     const int tid = threadIdx.x;
     const int n = cfg.n, m = cfg.m, d = cfg.d, D = cfg.D;
@@ -46,13 +46,16 @@ rollout_relift_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant_
     unsigned trig_mask = 0;                                     // bit j: sin x_j needed, bit 16 + j: cos x_j needed
     if (mono) {
         for (int f = tid; f < d; f += kRlBlock) {
-            unsigned packed = 0;
+            // the non-unit factors in order (a factor 1.0 multiplies exactly, so skipping it is bit-identical), their
+            // count in bits 24..26: most features are single states or products of two, not of four
+            unsigned packed = 0, cnt = 0;
             for (int q = 0; q < 4; q++) {
                 const unsigned code = cfg.terms[4 * f + q];
-                const unsigned slot = code == 0xFFu ? 0u : 1u + (code >> 6) * n + (code & 0x3Fu);
-                packed |= slot << (8 * q);
+                if (code == 0xFFu) continue;
+                packed |= (1u + (code >> 6) * n + (code & 0x3Fu)) << (6 * cnt);
+                cnt++;
             }
-            sslot[f] = packed;
+            sslot[f] = packed | (cnt << 24);
         }
         for (int f = 0; f < d; f++)                             // uniform, once per CTA
             for (int q = 0; q < 4; q++) {
@@ -114,11 +117,12 @@ rollout_relift_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant_
     // feature f (internal index) of the published state; same factor order as lift_feature
     auto feature = [&](int f) -> float {
         if (mono) {
-            const unsigned t = sslot[f];
-            float p = sv[(t & 0xFFu) * kRlBlock];
-            p = __fmul_rn(p, sv[((t >> 8) & 0xFFu) * kRlBlock]);
-            p = __fmul_rn(p, sv[((t >> 16) & 0xFFu) * kRlBlock]);
-            p = __fmul_rn(p, sv[(t >> 24) * kRlBlock]);
+            const unsigned t = sslot[f], cnt = t >> 24;                   // warp-uniform: no divergence
+            if (cnt == 0) return 1.0f;
+            float p = sv[(t & 0x3Fu) * kRlBlock];
+            if (cnt > 1) p = __fmul_rn(p, sv[((t >> 6) & 0x3Fu) * kRlBlock]);
+            if (cnt > 2) p = __fmul_rn(p, sv[((t >> 12) & 0x3Fu) * kRlBlock]);
+            if (cnt > 3) p = __fmul_rn(p, sv[((t >> 18) & 0x3Fu) * kRlBlock]);
             return p;
         }
         if (f < n) return sv[(1 + cfg.perm[f]) * kRlBlock];
