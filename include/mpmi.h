@@ -64,9 +64,11 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
        MPMI_VARIANT_LAT_R4 = 64,        /* latency kernel: 4 rows per lane                    */
        MPMI_VARIANT_NO_TENSOR = 128,    /* d = 128: FP32 SIMT tile kernel instead of the 3xTF32
                                            tcgen05 kernel (results agree within the tolerances) */
-       MPMI_VARIANT_AFFINE = 256 };     /* noise-free linear model: x_k = a_k + G_k u (G_k tabulated at
+       MPMI_VARIANT_AFFINE = 256,     /* noise-free linear model: x_k = a_k + G_k u (G_k tabulated at
                                            create, a_k per tick): n*m instead of d*(d+m) FMAs per
                                            sample-step; ignored with noise or the re-lift model   */
+       MPMI_VARIANT_NO_PREDICT = 512 }; /* d > 32: walk the candidates in input-box-cell order instead of
+                                           the order of their predicted life time                 */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:

@@ -7,8 +7,13 @@
 // box they fall in (cell = the top bits of the Philox words, row-major over the input dimensions):
 //   bin_hist_kernel    histogram of cells (one RED per candidate) + exclusive scan by the last CTA
 //   bin_scatter_kernel perm[cursor[cell]++] = local candidate index
+//   bin_predict_kernel (life-time order, below) replaces bin_hist_kernel: keys + histogram + scan
 // The rollout kernel then walks perm, so a warp owns candidates of the same cell.  The candidate SET,
 // every key and hence the result are unchanged (keys carry the original index).
+// Life-time order (persistent tile kernels, d > 32): in a 3-D input box cubic cells leave a tile of 128 candidates
+// running 0.65 N*H tile-steps for 0.46 N*H candidate-steps; there the cell is instead the first-violation step
+// PREDICTED by the affine-in-u form x_k = a_k + G_k u (rollout_affine.cuh, n*m FMAs per step), longest first, so
+// that the candidates of a tile stop together.  The prediction only schedules: the dense rollout decides.
 #pragma once
 #include "mpmi_device.cuh"
 
@@ -23,9 +28,15 @@ struct BinArgs {
     int *cursor;              // ncells, written by the scan
     int *perm;                // nsamp
     unsigned *ticket;
+    int *keys;                // life-time order: predicted steps of the local candidates (cell = H - steps), or null
+    int H;
 };
 
 __device__ __forceinline__ int cell_of(const DevCfg &cfg, const BinArgs &b, long long gi, unsigned long long tick) {
+    if (b.keys) {                                            // predicted life time, longest first
+        const int st = b.keys[gi - cfg.shard_begin];
+        return b.H - (st < 0 ? 0 : st > b.H ? b.H : st);
+    }
     unsigned w[4];
     philox4x32_10((unsigned)gi, (unsigned)((unsigned long long)gi >> 32), (unsigned)tick, (unsigned)(tick >> 32),
                   cfg.seed_lo, cfg.seed_hi, w);
@@ -36,10 +47,8 @@ __device__ __forceinline__ int cell_of(const DevCfg &cfg, const BinArgs &b, long
     return cell;
 }
 
-__global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
-    const unsigned long long tick = b.tick_val;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < b.nsamp; i += (long long)gridDim.x * blockDim.x)
-        atomicAdd(&b.hist[cell_of(cfg, b, cfg.shard_begin + i, tick)], 1);
+// exclusive scan of hist -> cursor by the last CTA to arrive (256 threads); hist is cleared for the next tick
+__device__ __forceinline__ void bin_scan_last_cta(const BinArgs &b) {
     __shared__ bool last;
     __shared__ int warp_tot[8];
     __threadfence();
@@ -85,10 +94,83 @@ __global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ D
     if (threadIdx.x == 0) *b.ticket = 0u;
 }
 
+__global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
+    const unsigned long long tick = b.tick_val;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < b.nsamp; i += (long long)gridDim.x * blockDim.x) {
+        const int cell = cell_of(cfg, b, cfg.shard_begin + i, tick);
+        if (b.keys) {
+            // few cells, and one of them (life = H) may hold most candidates: one RED per warp and cell
+            const unsigned peers = __match_any_sync(__activemask(), cell);
+            if ((threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&b.hist[cell], __popc(peers));
+        } else {
+            atomicAdd(&b.hist[cell], 1);
+        }
+    }
+    bin_scan_last_cta(b);
+}
+
+// Life-time keys and their histogram in one pass: thread = candidate, x_k = a_k + G_k u from the [k][1 + m][NP] table
+// in shared memory (a_k: affine_base_kernel of this tick, G_k: mpmi_create), first violation -> keys[i]; then the same
+// last-CTA scan as bin_hist_kernel.  The warp leaves the horizon loop once all its candidates are predicted dead.
+template <int NP>
+__global__ void __launch_bounds__(256) bin_predict_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
+    static_assert(NP == 4 || NP == 8 || NP == 16, "padded physical dim");
+    extern __shared__ __align__(16) float sag[];
+    const int m = cfg.m, H = b.H, stride = (1 + m) * NP;
+    for (int e = threadIdx.x; e < H * stride; e += 256) {
+        const int k = e / stride, c = (e % stride) / NP, j = e % NP;
+        sag[e] = c == 0 ? cfg.aff_a[k * NP + j] : cfg.aff_g[(k * m + (c - 1)) * NP + j];
+    }
+    __syncthreads();
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    const float none[kMaxM] = {0.f, 0.f, 0.f, 0.f};
+    float u[kMaxM];
+    sample_u(cfg, cfg.shard_begin + (i < b.nsamp ? i : 0), b.tick_val, none, u);
+    const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
+    bool alive = i < b.nsamp;
+    int steps = 0;
+    for (int k = 0; k < H; k++) {
+        if (!__any_sync(0xffffffffu, alive)) break;
+        const float *row = sag + k * stride;
+        float x[NP];
+#pragma unroll
+        for (int j = 0; j < NP; j += 4) {
+            float4 v = *reinterpret_cast<const float4 *>(row + j);
+#pragma unroll
+            for (int q = 0; q < kMaxM; q++) {
+                if (q < m) {
+                    const float4 g = *reinterpret_cast<const float4 *>(row + (1 + q) * NP + j);
+                    v.x = __fmaf_rn(g.x, u[q], v.x); v.y = __fmaf_rn(g.y, u[q], v.y);
+                    v.z = __fmaf_rn(g.z, u[q], v.z); v.w = __fmaf_rn(g.w, u[q], v.w);
+                }
+            }
+            x[j] = v.x; x[j + 1] = v.y; x[j + 2] = v.z; x[j + 3] = v.w;
+        }
+        alive = alive && safe_check<NP>(cfg, x, nbox);
+        steps += alive ? 1 : 0;
+    }
+    if (i < b.nsamp) {
+        b.keys[i] = steps;
+        const int cell = H - steps;
+        const unsigned peers = __match_any_sync(__activemask(), cell);
+        if ((threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&b.hist[cell], __popc(peers));
+    }
+    bin_scan_last_cta(b);
+}
+
 __global__ void __launch_bounds__(256) bin_scatter_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
     const unsigned long long tick = b.tick_val;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < b.nsamp; i += (long long)gridDim.x * blockDim.x) {
-        const int pos = atomicAdd(&b.cursor[cell_of(cfg, b, cfg.shard_begin + i, tick)], 1);
+        const int cell = cell_of(cfg, b, cfg.shard_begin + i, tick);
+        int pos = 0;
+        if (b.keys) {
+            const unsigned peers = __match_any_sync(__activemask(), cell);
+            const int lead = __ffs(peers) - 1, lane = threadIdx.x & 31;
+            if (lane == lead) pos = atomicAdd(&b.cursor[cell], __popc(peers));
+            pos = __shfl_sync(peers, pos, lead) + __popc(peers & ((1u << lane) - 1u));
+        } else {
+            pos = atomicAdd(&b.cursor[cell], 1);
+        }
         b.perm[pos] = (int)i;
     }
 }

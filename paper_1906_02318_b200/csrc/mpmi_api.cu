@@ -38,7 +38,7 @@ struct mpmi_ctx {
     KernFn k_batch_dump = nullptr;
     float *d_affA = nullptr, *d_affG = nullptr;
     cudaGraphNode_t n_base = nullptr;
-    float *d_KTa = nullptr, *d_W = nullptr, *d_b = nullptr;
+    float *d_KTa = nullptr, *d_W = nullptr, *d_b = nullptr, *d_affM = nullptr;
     uint8_t *d_terms = nullptr;
     TickState *d_state = nullptr;
     mpmi_result *h_res = nullptr, *d_res_mapped = nullptr;   // pinned + mapped: the tick kernel writes the result here
@@ -58,6 +58,10 @@ struct mpmi_ctx {
     BinArgs bin{};
     int *d_hist = nullptr, *d_cursor = nullptr, *d_perm = nullptr;
     unsigned *d_bin_ticket = nullptr;
+    // life-time order (binning.cuh): predicted steps of the local sampled candidates from the affine form
+    bool predict = false;
+    int *d_pred = nullptr;
+    const void *k_pred = nullptr;    // bin_predict_kernel<aff_np>
     std::string err;
 };
 
@@ -196,10 +200,15 @@ void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cuda
 }
 void launch_base(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {      // a_k = C K^k Psi(x_t) of the affine path
     void *args[2] = {(void *)&c->dc, (void *)&a};
-    cudaLaunchKernel((const void *)c->k_base, dim3(1), dim3((unsigned)c->dc.D), args, 0, s);
+    cudaLaunchKernel((const void *)c->k_base, dim3((unsigned)c->dc.H), dim3(128), args, 0, s);
 }
 
 // one tick on stream s: [cell histogram + scan, scatter] (large Philox sets only) -> fused tick kernel
+const void *pick_predict(int np) {
+    return np == 4 ? (const void *)bin_predict_kernel<4> : np == 8 ? (const void *)bin_predict_kernel<8> : (const void *)bin_predict_kernel<16>;
+}
+unsigned pred_smem(const mpmi_ctx *c) { return (unsigned)(c->dc.H * (1 + c->dc.m) * c->dc.aff_np * 4); }
+
 void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
     if (c->binning) {
         BinArgs b = c->bin;
@@ -207,7 +216,13 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         long long g = (b.nsamp + 255) / 256;
         const long long gmax = 8LL * c->sm_count;
         const unsigned grid = (unsigned)(g < gmax ? g : gmax);
-        bin_hist_kernel<<<grid, 256, 0, s>>>(c->dc, b);
+        if (c->predict) {        // a_k for this x_t, then predicted life times (keys) + their histogram + scan
+            launch_base(c, a, s);
+            void *pargs[2] = {(void *)&c->dc, (void *)&b};
+            cudaLaunchKernel(c->k_pred, dim3((unsigned)g), dim3(256), pargs, pred_smem(c), s);
+        } else {
+            bin_hist_kernel<<<grid, 256, 0, s>>>(c->dc, b);
+        }
         bin_scatter_kernel<<<grid, 256, 0, s>>>(c->dc, b);
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
@@ -231,7 +246,13 @@ void tick_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
 void base_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
     args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
-    p->func = (void *)c->k_base; p->gridDim = dim3(1); p->blockDim = dim3((unsigned)c->dc.D); p->kernelParams = args;
+    p->func = (void *)c->k_base; p->gridDim = dim3((unsigned)c->dc.H); p->blockDim = dim3(128); p->kernelParams = args;
+}
+void pred_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->gb;
+    p->func = (void *)c->k_pred; p->gridDim = dim3((unsigned)((c->bin.nsamp + 255) / 256)); p->blockDim = dim3(256);
+    p->sharedMemBytes = pred_smem(c); p->kernelParams = args;
 }
 void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
@@ -254,8 +275,15 @@ int build_graph(mpmi_ctx *c) {
         const long long gmax = 8LL * c->sm_count;
         c->bin_grid = (unsigned)(g < gmax ? g : gmax);
         c->ga.perm = c->d_perm; c->ga.nsamp = c->gb.nsamp;
-        bin_node_params(c, false, &p, args);
-        CU(c, cudaGraphAddKernelNode(&c->n_hist, c->graph, nullptr, 0, &p));
+        if (c->predict) {                        // base -> prediction (keys + histogram + scan) -> scatter -> tick
+            base_node_params(c, &p, args);
+            CU(c, cudaGraphAddKernelNode(&c->n_base, c->graph, nullptr, 0, &p));
+            pred_node_params(c, &p, args);
+            CU(c, cudaGraphAddKernelNode(&c->n_hist, c->graph, &c->n_base, 1, &p));
+        } else {
+            bin_node_params(c, false, &p, args);
+            CU(c, cudaGraphAddKernelNode(&c->n_hist, c->graph, nullptr, 0, &p));
+        }
         bin_node_params(c, true, &p, args);
         CU(c, cudaGraphAddKernelNode(&c->n_scatter, c->graph, &c->n_hist, 1, &p));
         dep = c->n_scatter;
@@ -296,10 +324,11 @@ void mpmi_destroy(mpmi_ctx *c) {
     if (c->pending) cudaStreamSynchronize(c->pending_stream);
     if (c->exec) cudaGraphExecDestroy(c->exec);
     if (c->graph) cudaGraphDestroy(c->graph);
-    cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
+    cudaFree(c->d_affM); cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
     cudaFree(c->d_state);
     slot_release(c->kslot);
     cudaFree(c->d_affA); cudaFree(c->d_affG);
+    cudaFree(c->d_pred);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_res);
     delete c;
@@ -465,9 +494,10 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             for (int t = 0; t < total; t++) c->bin.bits[t % m]++;
             c->bin.ncells = 1 << total;
             c->bin.nsamp = nsamp;
-            CUC(cudaMalloc(&c->d_hist, sizeof(int) * c->bin.ncells));
-            CUC(cudaMemset(c->d_hist, 0, sizeof(int) * c->bin.ncells));
-            CUC(cudaMalloc(&c->d_cursor, sizeof(int) * c->bin.ncells));
+            const size_t ncell_alloc = (size_t)(c->bin.ncells > cfg->H + 1 ? c->bin.ncells : cfg->H + 1);   // (life-time order: H + 1 cells)
+            CUC(cudaMalloc(&c->d_hist, sizeof(int) * ncell_alloc));
+            CUC(cudaMemset(c->d_hist, 0, sizeof(int) * ncell_alloc));
+            CUC(cudaMalloc(&c->d_cursor, sizeof(int) * ncell_alloc));
             CUC(cudaMalloc(&c->d_perm, sizeof(int) * nsamp));
             CUC(cudaMalloc(&c->d_bin_ticket, sizeof(unsigned)));
             CUC(cudaMemset(c->d_bin_ticket, 0, sizeof(unsigned)));
@@ -547,38 +577,74 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     }
     c->bsmem = c->smem;
     c->bpersistent = c->variant == 2 || c->variant == 4;
-    if ((cfg->variant & MPMI_VARIANT_AFFINE) && cfg->model == MPMI_MODEL_LINEAR && !noise && c->k_tick && c->k_batch) {
-        // x_k = a_k + G_k u: tabulate G_k = C S_k B, S_k = sum_{i<k} K^i, in FP64 (T_1 = B, T_{k+1} = K T_k + B)
-        const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16, Hh = cfg->H;
-        const size_t aff_smem = (size_t)Hh * (1 + m) * NPn * sizeof(float);
-        if (aff_smem <= 200 * 1024) {
-            std::vector<double> T((size_t)d * m), Tn((size_t)d * m);
-            std::vector<float> G((size_t)Hh * m * NPn, 0.f);
-            for (int r = 0; r < d; r++) for (int j = 0; j < m; j++) T[(size_t)r * m + j] = cfg->B[(size_t)r * m + j];
-            for (int k = 0; k < Hh; k++) {
-                for (int j = 0; j < m; j++)
-                    for (int q = 0; q < n; q++) G[((size_t)k * m + j) * NPn + q] = (float)T[(size_t)perm[q] * m + j];
-                for (int r = 0; r < d; r++)
-                    for (int j = 0; j < m; j++) {
-                        double sacc = cfg->B[(size_t)r * m + j];
-                        for (int q = 0; q < d; q++) sacc += (double)cfg->K[(size_t)r * d + q] * T[(size_t)q * m + j];
-                        Tn[(size_t)r * m + j] = sacc;
-                    }
-                T.swap(Tn);
-            }
-            CUC(cudaMalloc(&c->d_affG, G.size() * sizeof(float)));
-            CUC(cudaMemcpy(c->d_affG, G.data(), G.size() * sizeof(float), cudaMemcpyHostToDevice));
-            CUC(cudaMalloc(&c->d_affA, (size_t)Hh * NPn * sizeof(float)));
-            CUC(cudaMemset(c->d_affA, 0, (size_t)Hh * NPn * sizeof(float)));
-            dc.aff_g = c->d_affG; dc.aff_a = c->d_affA; dc.aff_np = NPn;
-            c->affine = true; c->variant = 6;
-            c->k_base = mpmi_pick_affine_base(D);
-            c->k_tick = mpmi_pick_affine(NPn, MODE_TICK);
-            c->k_batch_aff = mpmi_pick_affine(NPn, MODE_BATCH);
-            c->block = 256; c->cand_per_block = 256; c->smem = (int)aff_smem;
-            CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
-            CUC(cudaFuncSetAttribute((const void *)c->k_batch_aff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+    // x_k = a_k + G_k u: tabulate G_k = C S_k B, S_k = sum_{i<k} K^i, in FP64 (T_1 = B, T_{k+1} = K T_k + B); a_k comes per tick
+    // from affine_base_kernel.  Used by the affine variant and by the life-time order of the tile kernels.
+    const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16;
+    const size_t aff_smem = (size_t)cfg->H * (1 + m) * NPn * sizeof(float);
+    auto build_affine = [&]() -> int {
+        const int Hh = cfg->H;
+        std::vector<double> T((size_t)d * m), Tn((size_t)d * m);
+        std::vector<float> G((size_t)Hh * m * NPn, 0.f);
+        for (int r = 0; r < d; r++) for (int j = 0; j < m; j++) T[(size_t)r * m + j] = cfg->B[(size_t)r * m + j];
+        for (int k = 0; k < Hh; k++) {
+            for (int j = 0; j < m; j++)
+                for (int q = 0; q < n; q++) G[((size_t)k * m + j) * NPn + q] = (float)T[(size_t)perm[q] * m + j];
+            for (int r = 0; r < d; r++)
+                for (int j = 0; j < m; j++) {
+                    double sacc = cfg->B[(size_t)r * m + j];
+                    for (int q = 0; q < d; q++) sacc += (double)cfg->K[(size_t)r * d + q] * T[(size_t)q * m + j];
+                    Tn[(size_t)r * m + j] = sacc;
+                }
+            T.swap(Tn);
         }
+        // rows of C K^k in the internal order of KTa: R_1 = first n rows of K, R_{k+1} = R_k K
+        std::vector<float> Mt((size_t)Hh * NPn * D, 0.f);
+        {
+            std::vector<double> R((size_t)n * D, 0.0), Rn((size_t)n * D);
+            for (int q = 0; q < n; q++) for (int cc = 0; cc < D; cc++) R[(size_t)q * D + cc] = KTa[(size_t)cc * D + q];
+            for (int k = 0; k < Hh; k++) {
+                for (int q = 0; q < n; q++) for (int cc = 0; cc < D; cc++) Mt[((size_t)k * NPn + q) * D + cc] = (float)R[(size_t)q * D + cc];
+                if (k + 1 == Hh) break;
+                std::fill(Rn.begin(), Rn.end(), 0.0);
+                for (int q = 0; q < n; q++)
+                    for (int r = 0; r < D; r++) {
+                        const double v = R[(size_t)q * D + r];
+                        if (v != 0.0) for (int cc = 0; cc < D; cc++) Rn[(size_t)q * D + cc] += v * (double)KTa[(size_t)cc * D + r];
+                    }
+                R.swap(Rn);
+            }
+        }
+        CU(c, cudaMalloc(&c->d_affM, Mt.size() * sizeof(float)));
+        CU(c, cudaMemcpy(c->d_affM, Mt.data(), Mt.size() * sizeof(float), cudaMemcpyHostToDevice));
+        dc.aff_m = c->d_affM;
+        CU(c, cudaMalloc(&c->d_affG, G.size() * sizeof(float)));
+        CU(c, cudaMemcpy(c->d_affG, G.data(), G.size() * sizeof(float), cudaMemcpyHostToDevice));
+        CU(c, cudaMalloc(&c->d_affA, (size_t)Hh * NPn * sizeof(float)));
+        CU(c, cudaMemset(c->d_affA, 0, (size_t)Hh * NPn * sizeof(float)));
+        dc.aff_g = c->d_affG; dc.aff_a = c->d_affA; dc.aff_np = NPn;
+        c->k_base = mpmi_pick_affine_base(D);
+        c->k_batch_aff = mpmi_pick_affine(NPn, MODE_BATCH);
+        CU(c, cudaFuncSetAttribute((const void *)c->k_batch_aff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+        return MPMI_OK;
+    };
+    if ((cfg->variant & MPMI_VARIANT_AFFINE) && cfg->model == MPMI_MODEL_LINEAR && !noise && c->k_tick && c->k_batch &&
+        aff_smem <= 200 * 1024) {
+        rc = build_affine();
+        if (rc != MPMI_OK) return bail(rc);
+        c->affine = true; c->variant = 6;
+        c->k_tick = mpmi_pick_affine(NPn, MODE_TICK);
+        c->block = 256; c->cand_per_block = 256; c->smem = (int)aff_smem;
+        CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+    } else if ((c->variant == 2 || c->variant == 4) && c->binning && cfg->model == MPMI_MODEL_LINEAR && !noise &&
+               !(cfg->variant & MPMI_VARIANT_NO_PREDICT) && aff_smem <= 200 * 1024 && c->k_tick && c->k_batch) {
+        // life-time order for the persistent tile kernels (binning.cuh): cells = predicted first-violation steps
+        rc = build_affine();
+        if (rc != MPMI_OK) return bail(rc);
+        CUC(cudaMalloc(&c->d_pred, sizeof(int) * c->bin.nsamp));
+        c->predict = true;
+        c->k_pred = pick_predict(NPn);
+        CUC(cudaFuncSetAttribute(c->k_pred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+        c->bin.keys = c->d_pred; c->bin.H = cfg->H; c->bin.ncells = cfg->H + 1;
     }
     if (!c->k_tick || !c->k_batch) { c->err = "no kernel for this (d, m)"; return bail(MPMI_ERR_UNSUPPORTED); }
     cudaFuncAttributes fa;
@@ -599,7 +665,7 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
     if ((c->variant == 2 || c->variant == 4) && o->blocks > c->sm_count) o->blocks = c->sm_count;
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
-    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0); o->uses_graph = 1;
+    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0) + (c->predict ? 1 : 0); o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;
     o->ncand_local = c->dc.shard_count;
     return MPMI_OK;
@@ -623,12 +689,12 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     cudaKernelNodeParams p; void *args[2];
     if (c->binning) {
         c->gb.tick_val = tick;
-        bin_node_params(c, false, &p, args);
+        if (c->predict) pred_node_params(c, &p, args); else bin_node_params(c, false, &p, args);
         CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_hist, &p));
         bin_node_params(c, true, &p, args);
         CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_scatter, &p));
     }
-    if (c->affine) {
+    if (c->affine || c->predict) {
         base_node_params(c, &p, args);
         CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_base, &p));
     }

@@ -39,6 +39,7 @@ struct DevCfg {
     // affine-in-u fast path (rollout_affine.cuh): x_k = a_k + G_k u
     float *aff_a;                   // device: H x aff_np, written per tick by affine_base_kernel
     const float *aff_g;             // device: H x m x aff_np, from mpmi_create (FP64 -> fp32)
+    const float *aff_m;             // device: H x aff_np x D, rows of C K^k (FP64 -> fp32)
     int aff_np;                     // padded physical dim: 4, 8 or 16
 };
 

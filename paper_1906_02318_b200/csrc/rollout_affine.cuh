@@ -4,8 +4,8 @@
 // is affine in the candidate input:
 //     x_k = C K^k z_0 + (C S_k B) u = a_k + G_k u,      S_k = sum_{i<k} K^i,   k = 1..H.
 // G_k (n x m per step) depends on the model only and is computed once, in FP64, by mpmi_create;
-// a_k (n per step) depends on x_t and is produced per tick by affine_base_kernel, which rolls the
-// zero-input trajectory in fp32 with one CTA (thread r keeps row r of K in registers).  The candidate
+// a_k (n per step) depends on x_t and is produced per tick by affine_base_kernel as (C K^k) Psi(x_t), with the
+// n rows of C K^k tabulated in FP64 by mpmi_create as well (H independent n x d products, one CTA each).  The candidate
 // kernel then needs n*m FMAs per sample-step instead of d*(d+m): the SAME states, flags and selection
 // as Algorithm 2 up to fp32 rounding, at ~d^2/(n m) times less arithmetic.  It is
 // an opt-in variant (MPMI_VARIANT_AFFINE) with its own metric; it is invalid with prediction noise or
@@ -16,31 +16,23 @@
 
 namespace mpmi {
 
-// ---- a_k = C K^k Psi(x_t), k = 1..H: one CTA of D threads, z in shared memory (ping-pong) ------------
+// ---- a_k = (C K^k) Psi(x_t), k = 1..H: CTA k, the n rows of C K^k (FP64 at create, cfg.aff_m) times z_0 ----------
+// (H dependent mat-vec steps in one CTA took 25 us; H independent n x d products take a launch.)
+constexpr int kAffBaseThreads = 128;
 template <int D>
-__global__ void __launch_bounds__(D) affine_base_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
-    __shared__ float sz[2][D];
-    const int r = threadIdx.x;
+__global__ void __launch_bounds__(kAffBaseThreads) affine_base_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
+    __shared__ float sz[D];
     const float *x0p = a.inline_inputs ? a.x0_val : a.x0;
-    float krow[D];                                              // K[r][c] = KTa[c][r]
-#pragma unroll
-    for (int c = 0; c < D; c++) krow[c] = __ldg(cfg.KTa + c * D + r);
-    sz[0][r] = lift_feature(cfg, r, x0p);
+    for (int f = threadIdx.x; f < D; f += kAffBaseThreads) sz[f] = lift_feature(cfg, f, x0p);
     __syncthreads();
-    const int NP = cfg.aff_np;
-    for (int k = 0; k < cfg.H; k++) {
-        const float *z = sz[k & 1];
-        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;           // four chains: the sum is latency-bound
+    const int NP = cfg.aff_np, k = blockIdx.x, lane = threadIdx.x & 31;
+    for (int q = threadIdx.x >> 5; q < NP; q += kAffBaseThreads / 32) {
+        const float *mrow = cfg.aff_m + ((size_t)k * NP + q) * D;
+        float s = 0.f;
+        for (int c = lane; c < D; c += 32) s = __fmaf_rn(__ldg(mrow + c), sz[c], s);
 #pragma unroll
-        for (int c = 0; c < D; c += 4) {
-            const float4 v = *reinterpret_cast<const float4 *>(z + c);
-            s0 = __fmaf_rn(krow[c], v.x, s0); s1 = __fmaf_rn(krow[c + 1], v.y, s1);
-            s2 = __fmaf_rn(krow[c + 2], v.z, s2); s3 = __fmaf_rn(krow[c + 3], v.w, s3);
-        }
-        const float zn = (s0 + s1) + (s2 + s3);
-        sz[(k + 1) & 1][r] = zn;
-        if (r < NP) cfg.aff_a[k * NP + r] = r < cfg.n ? zn : 0.f;
-        __syncthreads();
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) cfg.aff_a[k * NP + q] = q < cfg.n ? s : 0.f;
     }
 }
 

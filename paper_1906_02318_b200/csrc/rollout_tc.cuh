@@ -263,8 +263,11 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
             if (tile >= ntile) break;
 
             // ---- a1 + a2: this thread's candidate, its half of z_0 and (column half 0) its input
-            long long li = (long long)tile * kTcTile + row;
-            if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];       // spatially ordered walk
+            // ordered walk (longest first): the ragged last tile holds the injected u_h, which may well run the
+            // whole horizon -- it goes first instead of alone at the very end
+            const unsigned wtile = (MODE == MODE_TICK && a.perm) ? (tile == 0 ? ntile - 1 : tile - 1) : tile;
+            long long li = (long long)wtile * kTcTile + row;
+            if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];
             const bool valid = li < ncand && inputs_ok;
             bool alive = valid;
             int steps = 0;

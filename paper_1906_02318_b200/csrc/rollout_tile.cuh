@@ -86,8 +86,10 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
         if (batch >= nbatch) break;
 
         // ---- a1 + a2: lane i fills column i of the warp tile
-        long long li = batch * WC + col;
-        if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];   // spatially ordered walk
+        // ordered walk: the ragged last batch holds the injected u_h (often the full horizon): first, not last
+        const long long wbatch = (MODE == MODE_TICK && a.perm) ? (batch == 0 ? nbatch - 1 : batch - 1) : batch;
+        long long li = wbatch * WC + col;
+        if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];
         bool alive = li < ncand && inputs_ok;
         int steps = 0;
         {

@@ -260,6 +260,38 @@ def test_spatial_binning_changes_nothing(mp, name, N):
             assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
 
 
+@pytest.mark.parametrize("name,N,noise,tensor", [("C5", 40000, 0.0, True), ("C5", 20000, 0.0, False), ("C5", 9000, 0.02, True)])
+def test_life_time_order_changes_nothing(mp, name, N, noise, tensor):
+    """For the persistent tile kernels (d > 32) the pre-sort key is the first-violation step PREDICTED by the
+    affine form x_k = a_k + G_k u (longest first), so that the candidates of a tile stop together.  The
+    prediction only orders the walk: the result is identical to the cell order and to the index order."""
+    w = W.make(name, N=N)
+    if noise:
+        w.noise_sigma = noise
+    V = mp.mpmi
+    base = 0 if tensor else V.VARIANT_NO_TENSOR           # tcgen05 kernel / FP32 warp-tile kernel
+    plain = mp.Context(w, variant=base | V.VARIANT_NO_BINNING)
+    cells = mp.Context(w, variant=base | V.VARIANT_FORCE_BINNING | V.VARIANT_NO_PREDICT)
+    pred = mp.Context(w, variant=base | V.VARIANT_FORCE_BINNING)
+    assert pred.info()["variant"] == (4 if tensor else 2)
+    if noise:                                # measured: no gain once noise decides the life time -> cell order
+        assert pred.info()["launches_per_tick"] == 3
+    else:
+        assert pred.info()["binning_cells"] == w.H + 1 and pred.info()["launches_per_tick"] == 4
+    assert cells.info()["launches_per_tick"] == 3 and plain.info()["launches_per_tick"] == 1
+    o = _oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 4)
+    for i, (x0, uu, t) in enumerate(zip(x0s, uus, ticks)):
+        a = plain.step_sync(x0, uu, int(t)).as_dict(w.m)
+        for ctx in (cells, pred):
+            b = ctx.step_sync(x0, uu, int(t)).as_dict(w.m)
+            for k in ("index", "safe", "steps", "n_safe", "n_exec", "key", "dist"):
+                assert a[k] == b[k], (k, a[k], b[k])
+            assert np.array_equal(a["u"], b["u"])
+        if i < 2 and not noise:
+            assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
+
+
 def test_edge_cases(mp):
     w = W.make("C1", N=1)
     o = _oracle(w)
