@@ -112,41 +112,48 @@ __global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ D
 // Life-time keys and their histogram in one pass: thread = candidate, x_k = a_k + G_k u from the [k][1 + m][NP] table
 // in shared memory (a_k: affine_base_kernel of this tick, G_k: mpmi_create), first violation -> keys[i]; then the same
 // last-CTA scan as bin_hist_kernel.  The warp leaves the horizon loop once all its candidates are predicted dead.
-template <int NP>
+template <int NP, int M>
 __global__ void __launch_bounds__(256) bin_predict_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
     static_assert(NP == 4 || NP == 8 || NP == 16, "padded physical dim");
     extern __shared__ __align__(16) float sag[];
-    const int m = cfg.m, H = b.H, stride = (1 + m) * NP;
+    constexpr int stride = (1 + M) * NP;
+    const int H = b.H;
     for (int e = threadIdx.x; e < H * stride; e += 256) {
         const int k = e / stride, c = (e % stride) / NP, j = e % NP;
-        sag[e] = c == 0 ? cfg.aff_a[k * NP + j] : cfg.aff_g[(k * m + (c - 1)) * NP + j];
+        sag[e] = c == 0 ? cfg.aff_a[k * NP + j] : cfg.aff_g[(k * M + (c - 1)) * NP + j];
     }
-    __syncthreads();
     const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
     const float none[kMaxM] = {0.f, 0.f, 0.f, 0.f};
     float u[kMaxM];
     sample_u(cfg, cfg.shard_begin + (i < b.nsamp ? i : 0), b.tick_val, none, u);
-    const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
+    // branch-free safe test: dims without a box limit hold (-inf, +inf) in cfg, no annulus becomes [0, +inf].  (An infinite
+    // state in an unlimited dim is predicted unsafe here, the rollout kernels call it safe: the prediction only orders the walk.)
+    const float r2lo = cfg.annulus ? cfg.rmin2 : 0.f, r2hi = cfg.annulus ? cfg.rmax2 : __int_as_float(0x7f800000);
+    __syncthreads();
     bool alive = i < b.nsamp;
     int steps = 0;
+#pragma unroll 2
     for (int k = 0; k < H; k++) {
         if (!__any_sync(0xffffffffu, alive)) break;
-        const float *row = sag + k * stride;
+        const float4 *row = reinterpret_cast<const float4 *>(sag + k * stride);
         float x[NP];
 #pragma unroll
-        for (int j = 0; j < NP; j += 4) {
-            float4 v = *reinterpret_cast<const float4 *>(row + j);
+        for (int j = 0; j < NP / 4; j++) {
+            float4 v = row[j];
 #pragma unroll
-            for (int q = 0; q < kMaxM; q++) {
-                if (q < m) {
-                    const float4 g = *reinterpret_cast<const float4 *>(row + (1 + q) * NP + j);
-                    v.x = __fmaf_rn(g.x, u[q], v.x); v.y = __fmaf_rn(g.y, u[q], v.y);
-                    v.z = __fmaf_rn(g.z, u[q], v.z); v.w = __fmaf_rn(g.w, u[q], v.w);
-                }
+            for (int q = 0; q < M; q++) {
+                const float4 g = row[(1 + q) * (NP / 4) + j];
+                v.x = __fmaf_rn(g.x, u[q], v.x); v.y = __fmaf_rn(g.y, u[q], v.y);
+                v.z = __fmaf_rn(g.z, u[q], v.z); v.w = __fmaf_rn(g.w, u[q], v.w);
             }
-            x[j] = v.x; x[j + 1] = v.y; x[j + 2] = v.z; x[j + 3] = v.w;
+            x[4 * j] = v.x; x[4 * j + 1] = v.y; x[4 * j + 2] = v.z; x[4 * j + 3] = v.w;
         }
-        alive = alive && safe_check<NP>(cfg, x, nbox);
+        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
+        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
+        bool ok = alive && (r2 >= r2lo) && (r2 <= r2hi);
+#pragma unroll
+        for (int j = 0; j < NP; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
+        alive = ok;
         steps += alive ? 1 : 0;
     }
     if (i < b.nsamp) {

@@ -204,9 +204,12 @@ void launch_base(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {      // a_
 }
 
 // one tick on stream s: [cell histogram + scan, scatter] (large Philox sets only) -> fused tick kernel
-const void *pick_predict(int np) {
-    return np == 4 ? (const void *)bin_predict_kernel<4> : np == 8 ? (const void *)bin_predict_kernel<8> : (const void *)bin_predict_kernel<16>;
+template <int NP>
+const void *pick_predict_m(int m) {
+    return m == 1 ? (const void *)bin_predict_kernel<NP, 1> : m == 2 ? (const void *)bin_predict_kernel<NP, 2>
+         : m == 3 ? (const void *)bin_predict_kernel<NP, 3> : (const void *)bin_predict_kernel<NP, 4>;
 }
+const void *pick_predict(int np, int m) { return np == 4 ? pick_predict_m<4>(m) : np == 8 ? pick_predict_m<8>(m) : pick_predict_m<16>(m); }
 unsigned pred_smem(const mpmi_ctx *c) { return (unsigned)(c->dc.H * (1 + c->dc.m) * c->dc.aff_np * 4); }
 
 void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
@@ -642,7 +645,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         if (rc != MPMI_OK) return bail(rc);
         CUC(cudaMalloc(&c->d_pred, sizeof(int) * c->bin.nsamp));
         c->predict = true;
-        c->k_pred = pick_predict(NPn);
+        c->k_pred = pick_predict(NPn, m);
         CUC(cudaFuncSetAttribute(c->k_pred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
         c->bin.keys = c->d_pred; c->bin.H = cfg->H; c->bin.ncells = cfg->H + 1;
     }
