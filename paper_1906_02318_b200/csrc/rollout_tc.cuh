@@ -10,8 +10,9 @@
 // fp32 accumulator tile itself serves as the A operand Z_hi of the next step:
 //
 //   TMEM (512 columns x 128 lanes, lane = candidate):  D0 | D1 (ping-pong fp32 state / accumulator)
-//        | A_lo (128 cols) | U_hi (8) | U_lo (8)
-//   shared memory: K_hi and K_lo as K-major no-swizzle B operands ([K | B | 0], 128 x 136 fp32 each).
+//        | A_lo (128 cols) | U = [u_hi (4) | u_lo (4)]
+//   shared memory: K_hi and K_lo as K-major no-swizzle B operands ([K | B B], 128 x 136 fp32 each; the second copy of B
+//   is zero in the lo image, so the input costs two MMAs per step: U K_lo = u_hi B_lo, U K_hi = (u_hi + u_lo) B_hi).
 //
 // Warp roles: warps 0..7 are "state" warps -- warp e owns TMEM lanes 32*(e%4).. and columns
 // 64*(e/4)..: after every step they read the new state with tcgen05.ld (thread = one candidate,
@@ -37,6 +38,9 @@ constexpr int kTcD = 128;                         // padded lifted dim
 constexpr int kTcKD = 144;                        // contraction length: 128 state + 8 input columns (m <= 4, zero padded)
                                                   // + 8 noise columns (n <= 8; used by the NOISE instantiation only)
 constexpr int kTcTile = 128;                      // candidates per tile = TMEM lanes
+#ifndef MPMI_TC_KSPLIT
+#define MPMI_TC_KSPLIT 15
+#endif
 #ifndef MPMI_TC_STATE_WARPS
 #define MPMI_TC_STATE_WARPS 8
 #endif
@@ -47,7 +51,7 @@ constexpr int kTcLBO = 128;                       // bytes between 16-byte K chu
 constexpr int kTcSBO = (kTcKD / 4) * 128;         // bytes between 8-row groups
 constexpr int kTcImg = (kTcD / 8) * kTcSBO;       // bytes of one B-operand image (69,632)
 constexpr int kTcSmemBytes = 2 * kTcImg;
-constexpr uint32_t kTcColD0 = 0, kTcColD1 = 128, kTcColAlo = 256, kTcColUhi = 384, kTcColUlo = 392, kTcColNhi = 400, kTcColNlo = 408;
+constexpr uint32_t kTcColD0 = 0, kTcColD1 = 128, kTcColAlo = 256, kTcColU = 384, kTcColNhi = 392, kTcColNlo = 400;
 
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 // x_lo = x - x_hi (exact) has up to 13 significant bits and the tensor core keeps 11 by TRUNCATION, a bias
@@ -98,6 +102,9 @@ struct TcShared {
     unsigned stop_tile;
     unsigned warp_alive[4];
     float z0[kTcD];
+#ifdef MPMI_TC_DEBUG
+    long long dbg_wake;
+#endif
 };
 
 // sigma * eps of Algorithm 2 l.5 for the tensor-core kernel: the state lives in the accumulator, so the
@@ -142,11 +149,15 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     // ---- one-off: B-operand images [K | B | 0] split into hi / lo, TMEM, barriers, shared lift
     for (int e = tid; e < kTcD * kTcKD; e += kTcThreads) {
         const int r = e % kTcD, c = e / kTcD;                        // K[r][c] = KTa[c][r]; rows D.. are B's columns
-        const float v = c < kTcD + cfg.m ? cfg.KTa[c * kTcD + r] : (c >= 136 && r == c - 136) ? 1.f : 0.f;   // [K | B | 0 | noise selector]
-        const float hi = tf32_hi(v);
+        // columns 128..135 meet the A block [u_hi (4) | u_lo (4)]: B twice in the hi image (u_hi B_hi + u_lo B_hi), B_lo once
+        // in the lo image (u_hi B_lo) -- two MMAs per step for the input instead of three
+        const int cb = c - kTcD;
+        const bool bcol = cb >= 0 && cb < 8 && (cb & 3) < cfg.m;
+        const float v = c < kTcD ? cfg.KTa[c * kTcD + r] : bcol ? cfg.KTa[(kTcD + (cb & 3)) * kTcD + r]
+                      : (c >= 136 && r == c - 136) ? 1.f : 0.f;                                   // [K | B B | noise selector]
         const int off = (r >> 3) * kTcSBO + (c >> 2) * kTcLBO + (r & 7) * 16 + (c & 3) * 4;
-        *reinterpret_cast<float *>(smem_img + off) = hi;
-        *reinterpret_cast<uint32_t *>(smem_img + kTcImg + off) = tf32_lo(v);
+        *reinterpret_cast<float *>(smem_img + off) = tf32_hi(v);
+        *reinterpret_cast<uint32_t *>(smem_img + kTcImg + off) = (cb >= 4 && cb < 8) ? 0u : tf32_lo(v);
     }
     float u_h[kMaxM] = {0.f, 0.f, 0.f, 0.f};
     bool inputs_ok = true;
@@ -203,13 +214,16 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     else { mbar_wait(bar_alo, p_alo); p_alo ^= 1; }
                     fence_after_sync();
                     TCT(tw_full);
+#ifdef MPMI_TC_DEBUG
+                    if (s > 0) *reinterpret_cast<volatile long long *>(&sh.dbg_wake) = clock64();
+#endif
                     // The small products go first: the tensor core accumulates with truncation toward zero
                     // (measured), so terms added while the accumulator is still ~2^-11 |z| lose nothing that
                     // matters, and only the 17 accumulations of Z_hi * K_hi run at full magnitude.
                     if (s == 0 && !(sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3])) {
                         sh.stop_tile = tile; mbar_arrive(bar_full); break;                  // nothing valid in this tile
                     }
-                    constexpr int kSplit = 12;                             // k-blocks of group 1 issued before the hand-back wait
+                    constexpr int kSplit = MPMI_TC_KSPLIT;                 // k-blocks of group 1 issued before the hand-back wait
 #pragma unroll
                     for (int kk = 0; kk < kSplit; kk++)                    // Z_hi * K_lo  (Z_hi = the fp32 state itself)
                         mma_tf32_ts(dnxt, dcur + 8 * kk, dlo + kk * kstep, idesc, kk > 0);
@@ -223,15 +237,15 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     }
                     TCT(tw_alo);
 #pragma unroll
-                    for (int kk = kSplit; kk < 17; kk++)
-                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColUhi, dlo + kk * kstep, idesc, true);
+                    for (int kk = kSplit; kk < 17; kk++)                   // (k-block 16: u_hi * B_lo)
+                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColU, dlo + kk * kstep, idesc, true);
 #pragma unroll
-                    for (int kk = 0; kk < 17; kk++)                        // Z_lo * K_hi
-                        mma_tf32_ts(dnxt, kk < 16 ? tb + kTcColAlo + 8 * kk : tb + kTcColUlo, dhi + kk * kstep, idesc, true);
+                    for (int kk = 0; kk < 16; kk++)                        // Z_lo * K_hi
+                        mma_tf32_ts(dnxt, tb + kTcColAlo + 8 * kk, dhi + kk * kstep, idesc, true);
                     if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNlo, dhi + 17 * kstep, idesc, true);     // (sigma eps)_lo through the selector
 #pragma unroll
-                    for (int kk = 0; kk < 17; kk++)                        // Z_hi * K_hi
-                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColUhi, dhi + kk * kstep, idesc, true);
+                    for (int kk = 0; kk < 17; kk++)                        // Z_hi * K_hi  (k-block 16: (u_hi + u_lo) * B_hi)
+                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColU, dhi + kk * kstep, idesc, true);
                     if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + 17 * kstep, idesc, true);     // (sigma eps)_hi
                     mma_commit(bar_full);
                     TCT(ti_23);
@@ -257,6 +271,12 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
         const float qnan = __int_as_float(0x7fc00000);
         unsigned p_full = 0, p_tile = 0;
+#ifdef MPMI_TC_DEBUG
+        long long sw_wait = 0, sw_ld = 0, sw_math = 0, sw_st = 0, sw_n = 0, sw_skew = 0, sq = clock64();
+#define SWT(acc) do { long long t_ = clock64(); acc += t_ - sq; sq = t_; } while (0)
+#else
+#define SWT(acc) do {} while (0)
+#endif
         for (unsigned it = 0;; it++) {
             mbar_wait(bar_tile, p_tile); p_tile ^= 1;
             const unsigned tile = sh.tile[it & 1];
@@ -299,15 +319,15 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     tmem_st16(tlane + kTcColAlo + c0 + cc, lo);
                 }
                 if (hc == 0) {
-                    uint32_t uh[8], ul[8];
+                    static_assert(kMaxM <= 4, "input block: [u_hi (4) | u_lo (4)]");
+                    uint32_t uv[8];
 #pragma unroll
-                    for (int j = 0; j < 8; j++) {
+                    for (int j = 0; j < 4; j++) {
                         const float uj = j < kMaxM ? u[j < kMaxM ? j : 0] : 0.f;
-                        uh[j] = __float_as_uint(uj);
-                        ul[j] = tf32_lo(uj);
+                        uv[j] = __float_as_uint(uj);
+                        uv[4 + j] = tf32_lo(uj);
                     }
-                    tmem_st8(tlane + kTcColUhi, uh);
-                    tmem_st8(tlane + kTcColUlo, ul);
+                    tmem_st8(tlane + kTcColU, uv);
                     const bool any = __any_sync(0xffffffffu, alive);
                     if (lane == 0) sh.warp_alive[q] = any ? 1u : 0u;
                 }
@@ -321,8 +341,14 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
             // ---- a3 + a4: after MMA step s-1 the accumulator holds z_s; test it, split it, hand it back
             int s = 1;
             for (; s <= H; s++) {
+                SWT(sw_math);
                 mbar_wait(bar_full, p_full); p_full ^= 1;
                 fence_after_sync();
+                SWT(sw_wait);
+#ifdef MPMI_TC_DEBUG
+                sw_n++;
+                if (s > 1) sw_skew += clock64() - *reinterpret_cast<volatile long long *>(&sh.dbg_wake);
+#endif
                 if (*reinterpret_cast<volatile unsigned *>(&sh.stop_tile) == tile) break;
                 const uint32_t dcol = (s & 1) ? kTcColD1 : kTcColD0;
                 const bool was_alive = alive;
@@ -334,6 +360,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 uint32_t rp[16];                                         // the physical state sits in columns 0..15
                 if (dump && hc != 0) tmem_ld16(tlane + dcol, rp);
                 wait_ld();
+                SWT(sw_ld);
                 if (hc == 0 || dump) {
                     float x[NB];
 #pragma unroll
@@ -366,9 +393,11 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     }
                 }
                 if (s < H) {
+                    SWT(sw_math);
                     wait_st();
                     fence_before_sync();
                     mbar_arrive(bar_alo);
+                    SWT(sw_st);
                 }
             }
             if (dump && li < ncand) {                                    // states after the tile stopped: NaN
@@ -400,6 +429,11 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 }
             }
         }
+#ifdef MPMI_TC_DEBUG
+        if (blockIdx.x == 0 && lane == 0 && (warp == 0 || warp == 4) && sw_n > 0)
+            printf("state warp %d (clk/step): wait %lld ld %lld math+st-issue %lld wait_st+arrive %lld  wake after the MMA thread %lld  steps %lld\n",
+                   warp, sw_wait / sw_n, sw_ld / sw_n, sw_math / sw_n, sw_st / sw_n, sw_skew / sw_n, sw_n);
+#endif
     }
 
     // ---- teardown: all MMAs of this CTA have completed (the state warps waited for the last commit)

@@ -292,6 +292,39 @@ def test_life_time_order_changes_nothing(mp, name, N, noise, tensor):
             assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
 
 
+def test_life_time_order_on_device_and_shard_paths(mp):
+    """The prediction runs ahead of the rollout on every entry point, not only in the tick graph: mpmi_step_device and
+    two shards (each predicts and sorts its own candidates) + finalize give the result of the unordered context."""
+    w = W.make("C5", N=30000)
+    V = mp.mpmi
+    plain = mp.Context(w, variant=V.VARIANT_NO_BINNING)
+    pred = mp.Context(w, variant=V.VARIANT_FORCE_BINNING)
+    cut = 17001
+    sh = [mp.Context(w, shard=(0, cut), variant=V.VARIANT_FORCE_BINNING),
+          mp.Context(w, shard=(cut, w.N + 1 - cut), variant=V.VARIANT_FORCE_BINNING)]
+    for c in (pred, sh[0], sh[1]):
+        assert c.info()["binning_cells"] == w.H + 1
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    d_res = torch.zeros(56, dtype=torch.uint8, device="cuda")
+    d_parts = torch.zeros(2 * 24, dtype=torch.uint8, device="cuda")
+    s = torch.cuda.current_stream().cuda_stream
+    for x0, uu, t in zip(x0s, uus, ticks):
+        host = plain.step_sync(x0, uu, int(t)).as_dict(w.m)
+        dx, du = _dev(x0), _dev(uu)
+        pred.step_device(dx.data_ptr(), du.data_ptr(), int(t), s, d_res.data_ptr())
+        torch.cuda.synchronize()
+        dev = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=V.RESULT_DTYPE)[0]
+        for g in range(2):
+            sh[g].shard_step(dx.data_ptr(), du.data_ptr(), int(t), s, d_parts.data_ptr() + 24 * g)
+        sh[0].shard_finalize(d_parts.data_ptr(), 2, du.data_ptr(), int(t), s, d_res.data_ptr())
+        torch.cuda.synchronize()
+        shd = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=V.RESULT_DTYPE)[0]
+        for got in (dev, shd):
+            for k in ("index", "safe", "steps", "n_safe", "n_exec", "key", "dist"):
+                assert got[k] == host[k], (k, got[k], host[k])
+            assert np.array_equal(got["u"][: w.m], host["u"])
+
+
 def test_edge_cases(mp):
     w = W.make("C1", N=1)
     o = _oracle(w)
