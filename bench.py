@@ -181,7 +181,7 @@ def run_sweep(args, w_full, local):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     K_, W_ = args.steps, args.warmup
     rows = []
-    variant = (mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0) | (mp.mpmi.VARIANT_NO_PREDICT if args.no_predict else 0)
+    variant = (mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0) | (mp.mpmi.VARIANT_NO_PREDICT if args.no_predict else 0) | (mp.mpmi.VARIANT_TENSOR32 if args.tensor32 else 0)
     for lg in range(14, 21):
         w = W.make(args.workload, N=1 << lg)
         w.noise_sigma = args.noise; w.model_kind = 1 if args.relift else 0
@@ -240,6 +240,7 @@ def main():
                     help="BASELINE.json configs[3]: N = 2^14 .. 2^20 on the chosen workload, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
                     help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
+    ap.add_argument("--tensor32", action="store_true", help="d = 32, N >= 2^17: opt-in 3xTF32 tcgen05 kernel (flags outside the 1e-4 margin rule at large states; DESIGN.md section 6)")
     ap.add_argument("--no-predict", action="store_true", help="d > 32: pre-sort by input-box cell instead of by predicted life time")
     ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
     ap.add_argument("--bounds-scale", type=float, default=1.0,
@@ -285,7 +286,7 @@ def main():
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
     begin, count = shard_plan(w.N, 1, world, rank)             # the injected u_user (index N) goes to the last rank
     ctx = mp.Context(w, device=local, shard=(begin, count) if sharded else (0, 0),
-                     variant=(mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0) | (mp.mpmi.VARIANT_NO_PREDICT if args.no_predict else 0))
+                     variant=(mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0) | (mp.mpmi.VARIANT_NO_PREDICT if args.no_predict else 0) | (mp.mpmi.VARIANT_TENSOR32 if args.tensor32 else 0))
     info = ctx.info()
     stream = torch.cuda.current_stream().cuda_stream
     if args.dump:
@@ -472,6 +473,8 @@ def main():
                                + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else "")
                                + (f", prediction noise sigma={args.noise}" if args.noise else "")
                                + (", re-lift model" if args.relift else "")
+                               + (", OPT-IN tensor-core variant at d = 32 (trajectories within 1e-4; flags outside the 1e-4 margin rule "
+                                  "for ~1e-4 of the candidates: not the parity-green default)" if args.tensor32 and info["variant"] == 4 else "")
                                + (", affine-in-u fast path (NEXT-4: separate metric, 2nm flop per sample-step)" if info["variant"] == 6 else ""),
                    "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
                    "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if sharded else "single GPU",

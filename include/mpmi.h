@@ -67,8 +67,14 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
        MPMI_VARIANT_AFFINE = 256,     /* noise-free linear model: x_k = a_k + G_k u (G_k tabulated at
                                            create, a_k per tick): n*m instead of d*(d+m) FMAs per
                                            sample-step; ignored with noise or the re-lift model   */
-       MPMI_VARIANT_NO_PREDICT = 512 }; /* d > 32: walk the candidates in input-box-cell order instead of
+       MPMI_VARIANT_NO_PREDICT = 512,   /* d > 32: walk the candidates in input-box-cell order instead of
                                            the order of their predicted life time                 */
+       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32, >= 2^17 candidates: the 3xTF32 tcgen05 kernel with
+                                           N = 32 MMAs, four CTAs per SM (2.2 x the FP32 register kernel).
+                                           OPT-IN: its trajectories meet the 1e-4 relative tolerance, but the
+                                           tensor core accumulates with truncation, and where states reach
+                                           ~1e2 the flags of ~1e-4 of the candidates with safe-set margins of
+                                           1e-4 .. 2e-4 differ from the FP64 oracle's   */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:

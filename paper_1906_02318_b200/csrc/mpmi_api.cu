@@ -62,6 +62,7 @@ struct mpmi_ctx {
     bool predict = false;
     int *d_pred = nullptr;
     const void *k_pred = nullptr;    // bin_predict_kernel<aff_np>
+    int tc_ctas = 1;                 // persistent CTAs per SM (4 for the tensor-core kernel at D = 32)
     std::string err;
 };
 
@@ -85,6 +86,7 @@ __global__ void shard_finalise_kernel(const __grid_constant__ DevCfg cfg, const 
 namespace {
 
 constexpr long long kLatMaxCand = 24576;        // <= this many candidates: latency kernel (measured: 125 vs 155 us at 2^14, 210 vs 164 us at 2^15)
+constexpr long long kTc32MinCand = 1LL << 17;   // D = 32: tensor-core kernel from this many candidates (four CTAs per SM need >= 592 tiles to fill)
 
 thread_local std::string g_create_err;
 
@@ -114,7 +116,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
 KernFn mpmi_pick_relift(int n, int mode);
 KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
-KernFn mpmi_pick_tc_tick(int *smem, int *threads, int noise); KernFn mpmi_pick_tc_batch(int *smem, int *threads, int noise);
+KernFn mpmi_pick_tc_tick(int D, int *smem, int *threads, int *ctas_per_sm, int noise); KernFn mpmi_pick_tc_batch(int D, int *smem, int *threads, int *ctas_per_sm, int noise);
 KernFn mpmi_pick_lat_8(int M, int R); KernFn mpmi_pick_lat_16(int M, int R); KernFn mpmi_pick_lat_32(int M, int R);
 namespace {
 KernFn pick_reg(int D, int M, int P, int mode, bool noise, int kconst = 1) {
@@ -183,7 +185,7 @@ void launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0,
     if (blocks < 1) blocks = 1;
     KArgs a = a0;
     if (persistent) {                            // persistent warp-tile / tensor-core kernel: one CTA per SM
-        if (blocks > c->sm_count) blocks = c->sm_count;
+        if (blocks > (long long)c->sm_count * c->tc_ctas) blocks = (long long)c->sm_count * c->tc_ctas;
         a.st = c->d_state; a.work = &c->d_state->work;
     }
     a.kslot = c->kslot;
@@ -236,7 +238,7 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
 unsigned grid_for(const mpmi_ctx *c, long long ncand) {
     long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
     if (blocks < 1) blocks = 1;
-    if ((c->variant == 2 || c->variant == 4) && blocks > c->sm_count) blocks = c->sm_count;
+    if ((c->variant == 2 || c->variant == 4) && blocks > (long long)c->sm_count * c->tc_ctas) blocks = (long long)c->sm_count * c->tc_ctas;
     return (unsigned)blocks;
 }
 
@@ -555,6 +557,19 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             c->k_tick = pick_lat(D, M, R);
             c->block = 64; c->cand_per_block = 64 / (D / R);     // D/R lanes per candidate
         }
+        // D = 32, large candidate sets, on request (MPMI_VARIANT_TENSOR32: its flags are not within the 1e-4 margin rule at
+        // large state magnitudes): the same 3xTF32 tcgen05 kernel as at d = 128, with N = 32 MMAs and four CTAs per SM
+        if (D == 32 && c->variant == 1 && (cfg->variant & MPMI_VARIANT_TENSOR32) && sc >= kTc32MinCand && (!noise || n <= 8) &&
+            !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY))) {
+            c->variant = 4; c->P = 1; c->k_batch_dump = nullptr;
+            int threads = 0;
+            c->k_tick = mpmi_pick_tc_tick(D, &c->smem, &threads, &c->tc_ctas, noise);
+            c->k_batch = mpmi_pick_tc_batch(D, &c->smem, &threads, &c->tc_ctas, noise);
+            c->block = threads; c->cand_per_block = 128;
+            c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
+            CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
+            CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
+        }
     } else {
         // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)
         // unless the caller asks for the FP32 SIMT tile kernel; d = 64 stays on the SIMT tile kernel
@@ -563,8 +578,8 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         if (tensor) {
             c->variant = 4;
             int threads = 0;
-            c->k_tick = mpmi_pick_tc_tick(&c->smem, &threads, noise);
-            c->k_batch = mpmi_pick_tc_batch(&c->smem, &threads, noise);
+            c->k_tick = mpmi_pick_tc_tick(D, &c->smem, &threads, &c->tc_ctas, noise);
+            c->k_batch = mpmi_pick_tc_batch(D, &c->smem, &threads, &c->tc_ctas, noise);
             c->block = threads; c->cand_per_block = 128;
         } else {
             c->variant = 2;
@@ -638,7 +653,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         c->k_tick = mpmi_pick_affine(NPn, MODE_TICK);
         c->block = 256; c->cand_per_block = 256; c->smem = (int)aff_smem;
         CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
-    } else if ((c->variant == 2 || c->variant == 4) && c->binning && cfg->model == MPMI_MODEL_LINEAR && !noise &&
+    } else if ((c->variant == 2 || c->variant == 4) && D > 32 && c->binning && cfg->model == MPMI_MODEL_LINEAR && !noise &&
                !(cfg->variant & MPMI_VARIANT_NO_PREDICT) && aff_smem <= 200 * 1024 && c->k_tick && c->k_batch) {
         // life-time order for the persistent tile kernels (binning.cuh): cells = predicted first-violation steps
         rc = build_affine();
@@ -665,8 +680,7 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     std::memset(o, 0, sizeof *o);
     o->d_pad = c->dc.D; o->variant = c->variant; o->cand_per_block = c->cand_per_block;
     o->threads_per_block = c->block;
-    o->blocks = (int)((c->dc.shard_count + c->cand_per_block - 1) / c->cand_per_block);
-    if ((c->variant == 2 || c->variant == 4) && o->blocks > c->sm_count) o->blocks = c->sm_count;
+    o->blocks = (int)grid_for(c, c->dc.shard_count);
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
     o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0) + (c->predict ? 1 : 0); o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;

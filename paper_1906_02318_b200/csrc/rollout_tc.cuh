@@ -34,24 +34,44 @@
 
 namespace mpmi {
 
-constexpr int kTcD = 128;                         // padded lifted dim
-constexpr int kTcKD = 144;                        // contraction length: 128 state + 8 input columns (m <= 4, zero padded)
-                                                  // + 8 noise columns (n <= 8; used by the NOISE instantiation only)
 constexpr int kTcTile = 128;                      // candidates per tile = TMEM lanes
+constexpr int kTcLBO = 128;                       // bytes between 16-byte K chunks (core matrices contiguous along K)
 #ifndef MPMI_TC_KSPLIT
 #define MPMI_TC_KSPLIT 15
 #endif
 #ifndef MPMI_TC_STATE_WARPS
 #define MPMI_TC_STATE_WARPS 8
 #endif
-constexpr int kTcStateWarps = MPMI_TC_STATE_WARPS;             // 4 lane quadrants x (2 or 4) column groups
-constexpr int kTcCols = 128 / (kTcStateWarps / 4);         // state columns per state-warp thread
-constexpr int kTcThreads = (kTcStateWarps + 1) * 32;
-constexpr int kTcLBO = 128;                       // bytes between 16-byte K chunks (core matrices contiguous along K)
-constexpr int kTcSBO = (kTcKD / 4) * 128;         // bytes between 8-row groups
-constexpr int kTcImg = (kTcD / 8) * kTcSBO;       // bytes of one B-operand image (69,632)
-constexpr int kTcSmemBytes = 2 * kTcImg;
-constexpr uint32_t kTcColD0 = 0, kTcColD1 = 128, kTcColAlo = 256, kTcColU = 384, kTcColNhi = 392, kTcColNlo = 400;
+// Geometry for padded lifted dim D = 128 (one CTA per SM, all 512 TMEM columns) and D = 32 (the same kernel with
+// N = 32 MMAs: a tile needs 3 D + 24 = 120 TMEM columns and 12 KB of operand images, so FOUR CTAs share an SM and
+// their step phases interleave -- measured: one CTA issues an M128 N32 K8 MMA every ~49 clk, four reach the 16 clk floor).
+template <int D>
+struct TcGeom {
+    static_assert(D == 128 || D == 32, "tensor-core rollout: D = 128 or 32");
+    static constexpr int kD = D;
+    static constexpr int kKB = D / 8;                              // k-blocks of the state
+    static constexpr int kKD = D + 16;                             // contraction length: D state + 8 input columns ([u_hi | u_lo], m <= 4)
+                                                                   // + 8 noise columns (n <= 8; used by the NOISE instantiation only)
+    static constexpr int kStateWarps = D == 128 ? MPMI_TC_STATE_WARPS : 4;   // 4 lane quadrants x column groups
+    static constexpr int kCols = D / (kStateWarps / 4);            // state columns per state-warp thread
+    static constexpr int kThreads = (kStateWarps + 1) * 32;
+    static constexpr int kSBO = (kKD / 4) * 128;                   // bytes between 8-row groups
+    static constexpr int kImg = (D / 8) * kSBO;                    // bytes of one B-operand image (69,632 at D = 128)
+    static constexpr int kSmemBytes = 2 * kImg;
+    static constexpr int kTmemCols = D == 128 ? 512 : 128;
+    static constexpr int kCtasPerSm = 512 / kTmemCols;
+    static constexpr int kSplit = D == 128 ? MPMI_TC_KSPLIT : kKB + 1;   // group-1 k-blocks issued before the hand-back wait
+    static constexpr uint32_t kColD0 = 0, kColD1 = D, kColAlo = 2 * D, kColU = 3 * D, kColNhi = 3 * D + 8, kColNlo = 3 * D + 16;
+};
+// the kernel body keeps the short names
+#define MPMI_TC_GEOM(D)                                                                                                     \
+    using G = TcGeom<D>;                                                                                                    \
+    constexpr int kTcD = G::kD, kTcKB = G::kKB, kTcKD = G::kKD, kTcStateWarps = G::kStateWarps, kTcCols = G::kCols,           \
+                  kTcThreads = G::kThreads, kTcSBO = G::kSBO, kTcImg = G::kImg;                                              \
+    constexpr uint32_t kTcColD0 = G::kColD0, kTcColD1 = G::kColD1, kTcColAlo = G::kColAlo, kTcColU = G::kColU,                \
+                       kTcColNhi = G::kColNhi, kTcColNlo = G::kColNlo;                                                       \
+    (void)kTcKB; (void)kTcKD; (void)kTcCols; (void)kTcThreads; (void)kTcSBO; (void)kTcImg; (void)kTcColD0; (void)kTcColD1;    \
+    (void)kTcColAlo; (void)kTcColU; (void)kTcColNhi; (void)kTcColNlo; (void)kTcStateWarps; (void)kTcD
 
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 // x_lo = x - x_hi (exact) has up to 13 significant bits and the tensor core keeps 11 by TRUNCATION, a bias
@@ -95,13 +115,14 @@ __device__ __forceinline__ bool safe_check_par(const DevCfg &cfg, const float (&
     return ok;
 }
 
+template <int D>
 struct TcShared {
     unsigned long long bar_full, bar_alo, bar_tile;
     uint32_t tmem_base;
     unsigned tile[2];
     unsigned stop_tile;
     unsigned warp_alive[4];
-    float z0[kTcD];
+    float z0[D];
 #ifdef MPMI_TC_DEBUG
     long long dbg_wake;
 #endif
@@ -109,8 +130,10 @@ struct TcShared {
 
 // sigma * eps of Algorithm 2 l.5 for the tensor-core kernel: the state lives in the accumulator, so the
 // noise enters the contraction as 8 extra A columns [sigma eps_hi | sigma eps_lo] against the selector rows of the K_hi
-// image (1.0 at (r = j, c = 136 + j): exact in TF32, its lo part is 0): z'_j += sigma eps_j through two more MMAs per step.
+// image (1.0 at (r = j, c = D + 8 + j): exact in TF32, its lo part is 0): z'_j += sigma eps_j through two more MMAs per step.
+template <int D>
 __device__ __forceinline__ void tc_noise_store(const DevCfg &cfg, long long gi, int k, unsigned long long tick, uint32_t tlane) {
+    MPMI_TC_GEOM(D);
     float g[8];                                                  // eps of the ORIGINAL dims 0..7
 #pragma unroll
     for (int q = 0; q < 2; q++) {
@@ -130,12 +153,13 @@ __device__ __forceinline__ void tc_noise_store(const DevCfg &cfg, long long gi, 
     tc::tmem_st8(tlane + kTcColNlo, nl);
 }
 
-template <int MODE, bool NOISE = false>
-__global__ void __launch_bounds__(kTcThreads, 1)
+template <int D, int MODE, bool NOISE = false>
+__global__ void __launch_bounds__(TcGeom<D>::kThreads, TcGeom<D>::kCtasPerSm)
 rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     using namespace tc;
+    MPMI_TC_GEOM(D);
     extern __shared__ __align__(1024) unsigned char smem_img[];      // K_hi image | K_lo image
-    __shared__ TcShared sh;
+    __shared__ TcShared<D> sh;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned long long tick = a.tick_val;
@@ -149,12 +173,12 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     // ---- one-off: B-operand images [K | B | 0] split into hi / lo, TMEM, barriers, shared lift
     for (int e = tid; e < kTcD * kTcKD; e += kTcThreads) {
         const int r = e % kTcD, c = e / kTcD;                        // K[r][c] = KTa[c][r]; rows D.. are B's columns
-        // columns 128..135 meet the A block [u_hi (4) | u_lo (4)]: B twice in the hi image (u_hi B_hi + u_lo B_hi), B_lo once
+        // columns D..D+7 meet the A block [u_hi (4) | u_lo (4)]: B twice in the hi image (u_hi B_hi + u_lo B_hi), B_lo once
         // in the lo image (u_hi B_lo) -- two MMAs per step for the input instead of three
-        const int cb = c - kTcD;
+        const int cb = c - kTcD;                                     // (at D = 128: columns 128..135 and 136..143)
         const bool bcol = cb >= 0 && cb < 8 && (cb & 3) < cfg.m;
         const float v = c < kTcD ? cfg.KTa[c * kTcD + r] : bcol ? cfg.KTa[(kTcD + (cb & 3)) * kTcD + r]
-                      : (c >= 136 && r == c - 136) ? 1.f : 0.f;                                   // [K | B B | noise selector]
+                      : (c >= kTcD + 8 && r == c - (kTcD + 8)) ? 1.f : 0.f;                       // [K | B B | noise selector]
         const int off = (r >> 3) * kTcSBO + (c >> 2) * kTcLBO + (r & 7) * 16 + (c & 3) * 4;
         *reinterpret_cast<float *>(smem_img + off) = tf32_hi(v);
         *reinterpret_cast<uint32_t *>(smem_img + kTcImg + off) = (cb >= 4 && cb < 8) ? 0u : tf32_lo(v);
@@ -167,7 +191,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     }
     if (shared_x0)
         for (int f = tid; f < kTcD; f += kTcThreads) sh.z0[f] = lift_feature(cfg, f, x0p);
-    if (warp == kTcStateWarps) tmem_alloc<512>(smem_u32(&sh.tmem_base));
+    if (warp == kTcStateWarps) tmem_alloc<G::kTmemCols>(smem_u32(&sh.tmem_base));
     if (tid == 0) {
         mbar_init(smem_u32(&sh.bar_full), 1);
         mbar_init(smem_u32(&sh.bar_alo), kTcStateWarps * 32);
@@ -223,10 +247,10 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     if (s == 0 && !(sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3])) {
                         sh.stop_tile = tile; mbar_arrive(bar_full); break;                  // nothing valid in this tile
                     }
-                    constexpr int kSplit = MPMI_TC_KSPLIT;                 // k-blocks of group 1 issued before the hand-back wait
+                    constexpr int kSplit = G::kSplit;                      // k-blocks of group 1 issued before the hand-back wait
 #pragma unroll
                     for (int kk = 0; kk < kSplit; kk++)                    // Z_hi * K_lo  (Z_hi = the fp32 state itself)
-                        mma_tf32_ts(dnxt, dcur + 8 * kk, dlo + kk * kstep, idesc, kk > 0);
+                        mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tb + kTcColU, dlo + kk * kstep, idesc, kk > 0);
                     TCT(ti_1);
                     if (s > 0) {                                           // state warps: z_s tested, Z_lo written
                         mbar_wait(bar_alo, p_alo); p_alo ^= 1;             // (its latency hides behind the queued MMAs)
@@ -237,16 +261,16 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     }
                     TCT(tw_alo);
 #pragma unroll
-                    for (int kk = kSplit; kk < 17; kk++)                   // (k-block 16: u_hi * B_lo)
-                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColU, dlo + kk * kstep, idesc, true);
+                    for (int kk = kSplit; kk < kTcKB + 1; kk++)            // (last k-block: u_hi * B_lo)
+                        mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tb + kTcColU, dlo + kk * kstep, idesc, true);
 #pragma unroll
-                    for (int kk = 0; kk < 16; kk++)                        // Z_lo * K_hi
+                    for (int kk = 0; kk < kTcKB; kk++)                     // Z_lo * K_hi
                         mma_tf32_ts(dnxt, tb + kTcColAlo + 8 * kk, dhi + kk * kstep, idesc, true);
-                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNlo, dhi + 17 * kstep, idesc, true);     // (sigma eps)_lo through the selector
+                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNlo, dhi + (kTcKB + 1) * kstep, idesc, true);     // (sigma eps)_lo through the selector
 #pragma unroll
-                    for (int kk = 0; kk < 17; kk++)                        // Z_hi * K_hi  (k-block 16: (u_hi + u_lo) * B_hi)
-                        mma_tf32_ts(dnxt, kk < 16 ? dcur + 8 * kk : tb + kTcColU, dhi + kk * kstep, idesc, true);
-                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + 17 * kstep, idesc, true);     // (sigma eps)_hi
+                    for (int kk = 0; kk < kTcKB + 1; kk++)                 // Z_hi * K_hi  (last k-block: (u_hi + u_lo) * B_hi)
+                        mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tb + kTcColU, dhi + kk * kstep, idesc, true);
+                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + (kTcKB + 1) * kstep, idesc, true);     // (sigma eps)_hi
                     mma_commit(bar_full);
                     TCT(ti_23);
                 }
@@ -332,7 +356,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     if (lane == 0) sh.warp_alive[q] = any ? 1u : 0u;
                 }
                 if (NOISE && hc == kTcStateWarps / 4 - 1)          // the last column group draws the noise of step 0
-                    tc_noise_store(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, 0, tick, tlane);
+                    tc_noise_store<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, 0, tick, tlane);
             }
             wait_st();
             fence_before_sync();
@@ -381,7 +405,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                         tmem_st8(tlane + kTcColAlo + c0 + cc, lo);
                     }
                     if (NOISE && hc == kTcStateWarps / 4 - 1)      // noise of MMA step s (it produces z_{s+1})
-                        tc_noise_store(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, s, tick, tlane);
+                        tc_noise_store<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, s, tick, tlane);
                 }
                 if (dump && li < ncand) {                                // a9: traj[(k*J + row)*Ncand + i], k = s-1
 #pragma unroll
@@ -439,7 +463,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     // ---- teardown: all MMAs of this CTA have completed (the state warps waited for the last commit)
     fence_before_sync();
     __syncthreads();
-    if (warp == kTcStateWarps) tc::tmem_dealloc<512>(tb);
+    if (warp == kTcStateWarps) tc::tmem_dealloc<G::kTmemCols>(tb);
     if (MODE == MODE_BATCH) {
         if (tid == 0) {                          // the last CTA to finish re-arms the work counter for the next launch
             __threadfence();
