@@ -420,7 +420,7 @@ def main():
     if os.path.exists(tj):
         for line in open(tj).read().splitlines()[1:]:
             f = line.split(",")
-            if f and f[0] == args.workload:
+            if f and f[0] == args.workload + ("-tensor32" if info["variant"] == 4 and w.d <= 32 else ""):
                 traffic = int(f[2])
     nominal_frac = nominal / K_ / max(world, 1) * flop / (total_ms * 1e-3 / K_) / 1e12 / FP32_PEAK_TFLOPS
     if info["variant"] == 4:
@@ -435,7 +435,7 @@ def main():
                     "peak_source": ("MEASURED_PEAKS.json bf16_tflops (burst; of measured)" if peaks else "fallback 1590 TFLOP/s bf16 (of fallback)")
                                    + " x 1.1/2.25 (nominal tf32:bf16) / 3 (3xTF32 split products per algorithmic flop)",
                     "kernel": "rollout_tc_kernel", "dtype": "3xTF32 (fp32 accumulate)",
-                    "tensor_tflops_executed": achieved * 3.0 * 136.0 / (w.d + w.m),
+                    "tensor_tflops_executed": achieved * 3.0 * (info["d_pad"] + 8.0) / (w.d + w.m),     # K padded to d_pad + one 8-wide input block
                     "fp32_alu_frac": achieved / FP32_PEAK_TFLOPS, "nominal_fp32_alu_frac": nominal_frac}
     else:
         roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
