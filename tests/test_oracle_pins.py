@@ -86,6 +86,39 @@ def test_grid_points_exact():
     assert np.array_equal(Oracle(w).sample(0, [5]), Oracle(w).sample(9, [5]))   # grid ignores tick
 
 
+def test_paper_race_car_grid_20x22x23(golden_dir):
+    """The paper's race-car sample set: N = 10,120 'equally spaced samples in all 3 input dimensions'
+     = 20 x 22 x 23 over heading [-1,1] x gas [0,1] x brake [-1,0]:
+    an asymmetric box with a different count per dimension.  Pinned against numpy's linspace / meshgrid
+    (endpoint-inclusive, dimension 0 slowest: DESIGN G3) and the row the paper prints for Eq. (2)."""
+    row = [l.split() for l in open(os.path.join(golden_dir, "eq2_printed.txt")) if l.startswith("race_car")][0]
+    counts = np.array([20, 22, 23], np.int32)
+    lo = np.array([-1, 0, -1], np.float32); hi = np.array([1, 1, 0], np.float32)
+    assert int(row[2]) == int(counts.prod()) == 10120
+    assert float(row[1]) == float((hi - lo).sum())                       # lambda* = 4 as printed (G7: a sum of lengths)
+    w = W.make("C5", N=10120, H=25)
+    w.sampler = 1; w.grid_counts = counts; w.u_lo = lo; w.u_hi = hi
+    o = Oracle(w, include_user=0)
+    u = o.sample(3, np.arange(10120))
+    axes = [np.linspace(float(lo[j]), float(hi[j]), int(counts[j])) for j in range(3)]
+    ref = np.stack(np.meshgrid(*axes, indexing="ij"), axis=-1).reshape(-1, 3)
+    assert np.abs(u.astype(np.float64) - ref).max() <= 2.0 ** -23        # fp32 rounding of the grid value
+    for j in range(3):
+        assert len(np.unique(u[:, j])) == counts[j]
+        assert u[:, j].min() == lo[j] and u[:, j].max() == hi[j]          # endpoints included, exactly
+    assert np.array_equal(u[0], lo) and np.array_equal(u[-1], hi)
+    assert u[1][2] > u[0][2] and u[1][0] == u[0][0] and u[23][1] > u[0][1] and u[22 * 23][0] > u[0][0]   # dim 0 slowest
+    # a tick on it: the selected input is a grid point (or the injected u_h) and lies in the box
+    o = Oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        r = o.step(x0, uu, int(t), detail=True)
+        assert np.all(r["u"] >= lo) and np.all(r["u"] <= hi)
+        assert 0 < r["n_safe"] < 10121                                    # a mixed set on this workload
+        if r["index"] < 10120:
+            assert np.array_equal(np.asarray(r["u"], np.float32), u[r["index"]])
+
+
 # ---------------------------------------------------------------- P9: lift -----------------------
 def test_lift_hand_values():
     w = W.make("C3", calibrated=False)

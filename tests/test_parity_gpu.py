@@ -624,6 +624,40 @@ def test_affine_flag_ignored_with_noise_or_relift(mp):
     assert mp.Context(w, variant=mp.mpmi.VARIANT_AFFINE).info()["variant"] == 5
 
 
+# ------------------------------------------------------------------ the paper's own race-car sample set ------------------
+def _paper_grid(relift=False):
+    """N = 10,120 = 20 x 22 x 23 equally spaced samples over heading [-1,1] x gas [0,1] x brake [-1,0], horizon 25
+    (PAPER.md:222, 242, 270), on the m = 3 model of C5 (the paper's trained race-car model is not available)."""
+    w = W.make("C5", N=10120, H=25)
+    w.sampler = 1; w.grid_counts = np.array([20, 22, 23], np.int32)
+    w.u_lo = np.array([-1, 0, -1], np.float32); w.u_hi = np.array([1, 1, 0], np.float32)
+    if relift:
+        w = G.scaled_bounds(w, 0.25); w.model_kind = 1
+    return w
+
+
+@pytest.mark.parametrize("variant,kernel", [(0, 4), (128, 2), (256, 6), ("relift", 5)])
+def test_paper_race_car_grid_tick(mp, variant, kernel):
+    """T3 on the paper's 3-D asymmetric grid through every kernel that serves d = 128: tcgen05, FP32 tile, affine, re-lift."""
+    w = _paper_grid(relift=(variant == "relift"))
+    ctx = mp.Context(w, variant=0 if variant == "relift" else variant)
+    assert ctx.info()["variant"] == kernel and ctx.info()["ncand_local"] == 10121
+    o = _oracle(w)
+    x0s, uus, ticks = W.tick_inputs(w, 10)
+    exact = 0; branches = set()
+    for x0, uu, t in zip(x0s, uus, ticks):
+        ref = o.step(x0, uu, int(t), detail=True)
+        r = ctx.step_sync(x0, uu, int(t)).as_dict(w.m)
+        ok, ex, why = accept_selection(r, ref, w.H)
+        assert ok, (why, r, {k: ref[k] for k in ("index", "safe", "steps", "dist")})
+        exact += ex
+        assert np.all(np.asarray(r["u"][:3]) >= w.u_lo) and np.all(np.asarray(r["u"][:3]) <= w.u_hi)
+        if (ref["margin_all"] > MARGIN).all():
+            assert r["n_safe"] == ref["n_safe"] and r["n_exec"] == ref["n_exec"]
+        branches.add("user" if (r["safe"] and r["dist"] == 0) else "intervene" if r["safe"] else "fallback")
+    assert exact >= 9 and "intervene" in branches, (exact, branches)
+
+
 # ------------------------------------------------------------------ d = 128: both kernels stay covered ------------------
 def test_fp32_tile_kernel_d128_parity(mp):
     """MPMI_VARIANT_NO_TENSOR keeps the FP32 SIMT warp-tile kernel reachable at d = 128: T1 / T2 and the same winner
