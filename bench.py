@@ -240,7 +240,7 @@ def main():
                     help="BASELINE.json configs[3]: N = 2^14 .. 2^20 on the chosen workload, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
                     help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
-    ap.add_argument("--tensor32", action="store_true", help="d = 32, N >= 2^17: opt-in 3xTF32 tcgen05 kernel (flags outside the 1e-4 margin rule at large states; DESIGN.md section 6)")
+    ap.add_argument("--tensor32", action="store_true", help="d = 32, N >= 2^17: opt-in verified tensor-core tick (3xTF32 tcgen05 rollout + FP32 second pass over the candidates near the boundary; DESIGN.md section 6)")
     ap.add_argument("--no-predict", action="store_true", help="d > 32: pre-sort by input-box cell instead of by predicted life time")
     ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
     ap.add_argument("--bounds-scale", type=float, default=1.0,
@@ -473,8 +473,8 @@ def main():
                                + (f", safe set scaled x{args.bounds_scale}" if args.bounds_scale != 1.0 else "")
                                + (f", prediction noise sigma={args.noise}" if args.noise else "")
                                + (", re-lift model" if args.relift else "")
-                               + (", OPT-IN tensor-core variant at d = 32 (trajectories within 1e-4; flags outside the 1e-4 margin rule "
-                                  "for ~1e-4 of the candidates: not the parity-green default)" if args.tensor32 and info["variant"] == 4 else "")
+                               + (", opt-in VERIFIED tensor-core tick at d = 32: 3xTF32 tcgen05 rollout, candidates that came near the safe-set boundary "
+                                  "are rolled again by the FP32 register kernel (same result as the FP32 tick; DESIGN.md section 6)" if args.tensor32 and info["variant"] == 4 else "")
                                + (", affine-in-u fast path (NEXT-4: separate metric, 2nm flop per sample-step)" if info["variant"] == 6 else ""),
                    "candidates_total": int(w.N + 1), "l2": "256 MB buffer written between timed iterations",
                    "parallelism": f"candidate shards x{world}, one 24-byte all-gather per tick" if sharded else "single GPU",

@@ -69,12 +69,14 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
                                            sample-step; ignored with noise or the re-lift model   */
        MPMI_VARIANT_NO_PREDICT = 512,   /* d > 32: walk the candidates in input-box-cell order instead of
                                            the order of their predicted life time                 */
-       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32, >= 2^17 candidates: the 3xTF32 tcgen05 kernel with
-                                           N = 32 MMAs, four CTAs per SM (2.2 x the FP32 register kernel).
-                                           OPT-IN: its trajectories meet the 1e-4 relative tolerance, but the
-                                           tensor core accumulates with truncation, and where states reach
-                                           ~1e2 the flags of ~1e-4 of the candidates with safe-set margins of
-                                           1e-4 .. 2e-4 differ from the FP64 oracle's   */
+       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32, >= 2^17 candidates: VERIFIED tensor-core tick.  The
+                                           3xTF32 tcgen05 kernel (N = 32 MMAs, four CTAs per SM) rolls all
+                                           candidates; every candidate whose state came within tau of the
+                                           safe-set boundary (tau ~ 6e-5 x the bounds, ~5 x the worst
+                                           3xTF32-vs-FP32 state difference) is rolled again by the FP32
+                                           register kernel, which merges its keys and finalises: flags and
+                                           winner are those of the FP32 tick.  mpmi_rollout_batch of such a
+                                           context runs the FP32 kernels             */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:
@@ -155,12 +157,12 @@ typedef struct {
     int32_t  d_pad;           /* internal padded lifted dim (zero rows / columns: exact)            */
     int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = warp-tile FFMA2 (d<=128),
                                  3 = latency kernel, 4 lanes per candidate (d<=32, small N),
-                                 4 = 3xTF32 tcgen05 tensor-core kernel (d_pad = 128),
+                                 4 = 3xTF32 tcgen05 tensor-core kernel (d_pad = 128; d_pad = 32 with MPMI_VARIANT_TENSOR32),
                                  5 = re-lift kernel (MPMI_MODEL_RELIFT), 6 = affine-in-u kernel       */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;
     int32_t  binning_cells;   /* 0 = candidates walked in index order; else cells of the spatial pre-sort */
-    int32_t  reserved;
+    int32_t  reserved;        /* verified tensor-core tick: candidates the last finished tick handed to the FP32 pass; else 0 */
     int64_t  ncand_local;     /* candidates this context rolls out per tick                         */
 } mpmi_info;
 

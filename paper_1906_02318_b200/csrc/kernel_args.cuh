@@ -23,6 +23,12 @@ struct KArgs {
     const int *perm;                      // device, spatial order of the local sampled candidates, or null
     long long nsamp;                      // sampled candidates of this shard (perm entries)
     unsigned *work;                       // device batch counter of the persistent tile kernel (zero between launches)
+    // verified tensor-core tick (D = 32): candidates that came within tau of the safe-set boundary in the 3xTF32 rollout are
+    // not keyed there but appended to `recheck`; the FP32 register kernel (recheck_mode = 1) rolls exactly those again,
+    // merges its keys into the same TickState and finalises the tick
+    int *recheck;                         // device, capacity = local candidates, or null
+    unsigned *recheck_count;              // device; zeroed by the CTA that finalises
+    int recheck_mode;                     // register kernel: 1 = walk recheck[0 .. *recheck_count) instead of the index space
     // batch
     const float *U;                       // device Ncand*m or null
     long long x0_count;

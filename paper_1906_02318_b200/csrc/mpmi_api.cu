@@ -63,6 +63,14 @@ struct mpmi_ctx {
     int *d_pred = nullptr;
     const void *k_pred = nullptr;    // bin_predict_kernel<aff_np>
     int tc_ctas = 1;                 // persistent CTAs per SM (4 for the tensor-core kernel at D = 32)
+    // verified tensor-core tick at D = 32: the tcgen05 kernel defers the candidates that came near the safe-set boundary
+    // to the FP32 register kernel, which merges them and finalises (kernel_args.cuh: recheck)
+    KernFn k_recheck = nullptr;
+    int *d_recheck = nullptr;
+    unsigned *d_recheck_count = nullptr;
+    unsigned recheck_grid = 0;
+    cudaGraphNode_t n_recheck = nullptr;
+    KArgs gr{};
     std::string err;
 };
 
@@ -232,7 +240,13 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
     if (c->affine) launch_base(c, a, s);
+    if (c->k_recheck) { a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; }
     launch(c, c->k_tick, c->dc.shard_count, a, s);
+    if (c->k_recheck) {                          // second pass: FP32 register kernel over the deferred candidates
+        a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1; a.kslot = c->kslot; a.work = nullptr;
+        void *args[2] = {(void *)&c->dc, (void *)&a};
+        cudaLaunchKernel((const void *)c->k_recheck, dim3(c->recheck_grid), dim3(kRegBlock), args, 0, s);
+    }
 }
 
 unsigned grid_for(const mpmi_ctx *c, long long ncand) {
@@ -266,9 +280,18 @@ void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **
     p->gridDim = dim3(c->bin_grid); p->blockDim = dim3(256); p->kernelParams = args;
 }
 
+void recheck_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
+    c->gr = c->ga;                               // same inputs, sequence number and result slot as the tick node
+    c->gr.perm = nullptr; c->gr.nsamp = 0; c->gr.work = nullptr; c->gr.recheck_mode = 1;
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->gr;
+    p->func = (void *)c->k_recheck; p->gridDim = dim3(c->recheck_grid); p->blockDim = dim3(kRegBlock); p->kernelParams = args;
+}
+
 int build_graph(mpmi_ctx *c) {
     c->ga = KArgs{};
     c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1; c->ga.kslot = c->kslot;
+    if (c->k_recheck) { c->ga.recheck = c->d_recheck; c->ga.recheck_count = c->d_recheck_count; }
     if (c->variant == 2 || c->variant == 4) c->ga.work = &c->d_state->work;
     c->tick_grid = grid_for(c, c->dc.shard_count);
     CU(c, cudaGraphCreate(&c->graph, 0));
@@ -302,6 +325,10 @@ int build_graph(mpmi_ctx *c) {
     }
     tick_node_params(c, &p, args);
     CU(c, cudaGraphAddKernelNode(&c->n_tick, c->graph, ndep ? deps : nullptr, ndep, &p));
+    if (c->k_recheck) {
+        recheck_node_params(c, &p, args);
+        CU(c, cudaGraphAddKernelNode(&c->n_recheck, c->graph, &c->n_tick, 1, &p));
+    }
     CU(c, cudaGraphInstantiate(&c->exec, c->graph, 0));
     return MPMI_OK;
 }
@@ -334,6 +361,7 @@ void mpmi_destroy(mpmi_ctx *c) {
     slot_release(c->kslot);
     cudaFree(c->d_affA); cudaFree(c->d_affG);
     cudaFree(c->d_pred);
+    cudaFree(c->d_recheck); cudaFree(c->d_recheck_count);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_res);
     delete c;
@@ -561,14 +589,21 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         // large state magnitudes): the same 3xTF32 tcgen05 kernel as at d = 128, with N = 32 MMAs and four CTAs per SM
         if (D == 32 && c->variant == 1 && (cfg->variant & MPMI_VARIANT_TENSOR32) && sc >= kTc32MinCand && (!noise || n <= 8) &&
             !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY))) {
-            c->variant = 4; c->P = 1; c->k_batch_dump = nullptr;
-            int threads = 0;
+            // The tick is VERIFIED: candidates whose 3xTF32 state came near the safe-set boundary are rolled again by the
+            // FP32 register kernel (2 candidates per thread), so flags and winner are those of the FP32 path.  The batch
+            // entry stays on the FP32 register kernels chosen above.
+            c->variant = 4;
+            int threads = 0, bs = 0, bt = 0, bc = 0;
             c->k_tick = mpmi_pick_tc_tick(D, &c->smem, &threads, &c->tc_ctas, noise);
-            c->k_batch = mpmi_pick_tc_batch(D, &c->smem, &threads, &c->tc_ctas, noise);
+            (void)mpmi_pick_tc_batch(D, &bs, &bt, &bc, noise);
             c->block = threads; c->cand_per_block = 128;
-            c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
             CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
-            CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
+            // the second pass sees a few 10^4 candidates: below ~2^19 the shared-memory model is the faster one (section 9 sweep)
+            c->k_recheck = pick_reg(D, M, 1, MODE_TICK, noise, 0);
+            c->recheck_grid = (unsigned)((sc + 2 * kRegBlock - 1) / (2 * kRegBlock));
+            CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc));
+            CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned)));
+            CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned)));
         }
     } else {
         // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)
@@ -593,8 +628,8 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
         }
     }
-    c->bsmem = c->smem;
-    c->bpersistent = c->variant == 2 || c->variant == 4;
+    c->bsmem = c->k_recheck ? 0 : c->smem;
+    c->bpersistent = (c->variant == 2 || c->variant == 4) && !c->k_recheck;
     // x_k = a_k + G_k u: tabulate G_k = C S_k B, S_k = sum_{i<k} K^i, in FP64 (T_1 = B, T_{k+1} = K T_k + B); a_k comes per tick
     // from affine_base_kernel.  Used by the affine variant and by the life-time order of the tile kernels.
     const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16;
@@ -682,9 +717,11 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->threads_per_block = c->block;
     o->blocks = (int)grid_for(c, c->dc.shard_count);
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
-    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0) + (c->predict ? 1 : 0); o->uses_graph = 1;
+    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0) + (c->predict ? 1 : 0) + (c->k_recheck ? 1 : 0); o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;
     o->ncand_local = c->dc.shard_count;
+    if (c->k_recheck)                            // candidates the last finished tick handed to the FP32 pass
+        cudaMemcpy(&o->reserved, &c->d_state->pad, sizeof(int), cudaMemcpyDeviceToHost);
     return MPMI_OK;
 }
 
@@ -717,6 +754,10 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     }
     tick_node_params(c, &p, args);
     CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_tick, &p));
+    if (c->k_recheck) {
+        recheck_node_params(c, &p, args);
+        CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_recheck, &p));
+    }
     CU(c, cudaGraphLaunch(c->exec, (cudaStream_t)stream));
     c->pending = true; c->pending_stream = (cudaStream_t)stream;
     c->err.clear();

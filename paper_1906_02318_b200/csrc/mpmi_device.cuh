@@ -242,7 +242,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                                                           unsigned n_safe, unsigned long long n_exec,
                                                           unsigned long long tick, const float (&u_h)[kMaxM],
                                                           TickState *st, mpmi_result *out, mpmi_partial *partial,
-                                                          unsigned seq = 0, unsigned *work = nullptr) {
+                                                          unsigned seq = 0, unsigned *work = nullptr, bool defer = false) {
     __shared__ unsigned long long s_key[kWarps];
     __shared__ unsigned s_safe[kWarps];
     __shared__ unsigned long long s_exec[kWarps];
@@ -261,13 +261,17 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
         for (int w = 1; w < kWarps; w++) {
             if (w * 32 < (int)blockDim.x) { k = s_key[w] < k ? s_key[w] : k; ns += s_safe[w]; ne += s_exec[w]; }
         }
-        atomicMin(&st->best_key, k);
+        if (k != kKeyNone) atomicMin(&st->best_key, k);
         if (ns) atomicAdd(&st->n_safe, ns);
-        atomicAdd(&st->n_exec, ne);
+        if (ne) atomicAdd(&st->n_exec, ne);
         __threadfence();
         const unsigned t = atomicAdd(&st->ticket, 1u);
         s_last = (t == gridDim.x - 1);
-        if (s_last) {
+        if (s_last && defer) {          // a later kernel of this tick merges its candidates and finalises: only re-arm the counters
+            st->ticket = 0u;
+            if (work) *work = 0u;
+            __threadfence();
+        } else if (s_last) {
             __threadfence();
             const unsigned long long bk = atomicMin(&st->best_key, kKeyNone);     // atomic read
             const unsigned long long tot_exec = atomicAdd(&st->n_exec, 0ull);
@@ -278,7 +282,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                 decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out, seq);
             }
             st->best_key = kKeyNone; st->n_exec = 0ull; st->n_safe = 0u; st->ticket = 0u;   // ready for next tick
-            if (work) *work = 0u;
+            if (work) { st->pad = *work; *work = 0u; }
             __threadfence();
         }
     }

@@ -115,6 +115,31 @@ __device__ __forceinline__ bool safe_check_par(const DevCfg &cfg, const float (&
     return ok;
 }
 
+// Verified tick (D = 32): did this state come within tau of the safe-set boundary (on either side)?  The 3xTF32 rollout is
+// within ~2e-5 relative of the FP32 one, so a candidate that never does has the same flags in both; one that does is
+// rolled again by the FP32 register kernel (kernel_args.cuh: recheck).  tau_box in state units, tau_ann2 in r^2 units.
+template <int NB>
+__device__ __forceinline__ bool near_boundary(const DevCfg &cfg, const float (&x)[NB], int nbox, float tau_box, float tau_ann2) {
+    bool nr = false;
+    if (nbox > 0) {
+        float m = box_slack<NB, 0, 2>(cfg, x);
+        if (nbox > 2) {
+            m = min_nan(m, box_slack<NB, 2, 4>(cfg, x));
+            if (nbox > 4) {
+                m = min_nan(m, box_slack<NB, 4, 8>(cfg, x));
+                if (nbox > 8) m = min_nan(m, box_slack<NB, 8, 16>(cfg, x));
+            }
+        }
+        nr = fabsf(m) < tau_box;
+    }
+    if (cfg.annulus) {
+        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
+        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
+        nr = nr || fabsf(fminf(__fsub_rn(r2, cfg.rmin2), __fsub_rn(cfg.rmax2, r2))) < tau_ann2;
+    }
+    return nr;
+}
+
 template <int D>
 struct TcShared {
     unsigned long long bar_full, bar_alo, bar_tile;
@@ -294,6 +319,19 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
         const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
         const float qnan = __int_as_float(0x7fc00000);
+        // verified tick: tau = 6e-5 x the size of the bounds (>= 5e-4).  Measured on C4 (|x| ~ 10, |z| ~ 130): the 3xTF32
+        // states drift from the FP32 ones by <= 1.5e-5 relative over H = 100 steps (flags differ from the oracle's only at
+        // margins <= 1.4e-4), so tau = 7.2e-4 there is ~5x the worst difference; ~3 % of the candidates take the second pass
+        const bool verify = (D == 32) && (MODE == MODE_TICK) && a.recheck != nullptr;
+        float tau_box = 5e-4f, tau_ann2 = 0.f;
+        if (verify) {
+            for (int j = 0; j < nbox && j < NB; j++) {
+                if (isfinite(cfg.blo[j])) tau_box = fmaxf(tau_box, 6e-5f * fabsf(cfg.blo[j]));
+                if (isfinite(cfg.bhi[j])) tau_box = fmaxf(tau_box, 6e-5f * fabsf(cfg.bhi[j]));
+            }
+            const float rmax = sqrtf(cfg.rmax2);
+            tau_ann2 = 2.f * rmax * fmaxf(5e-4f, 6e-5f * rmax);
+        }
         unsigned p_full = 0, p_tile = 0;
 #ifdef MPMI_TC_DEBUG
         long long sw_wait = 0, sw_ld = 0, sw_math = 0, sw_st = 0, sw_n = 0, sw_skew = 0, sq = clock64();
@@ -314,6 +352,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
             if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];
             const bool valid = li < ncand && inputs_ok;
             bool alive = valid;
+            bool near = false;
             int steps = 0;
             float u[kMaxM] = {0.f, 0.f, 0.f, 0.f};
             if (li < ncand) {
@@ -390,6 +429,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
 #pragma unroll
                     for (int j = 0; j < NB; j++) x[j] = __uint_as_float(hc == 0 ? r[j] : rp[j]);
                     alive = safe_check_par<NB>(cfg, x, nbox) && was_alive;
+                    if (verify) near = near || (was_alive && near_boundary<NB>(cfg, x, nbox, tau_box, tau_ann2));
                     steps += alive ? 1 : 0;
                 }
                 if (hc == 0) {
@@ -438,7 +478,20 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                         a.steps[li] = steps;
                         if (a.safe) a.safe[li] = steps == H ? 1 : 0;
                     }
-                } else if (valid) {                                      // a5: this candidate's key
+                }
+                bool push = false;
+                if (MODE == MODE_TICK && verify) {                       // near the boundary: the FP32 kernel decides (warp-aggregated append)
+                    push = valid && near;
+                    const unsigned mk = __ballot_sync(0xffffffffu, push);
+                    if (mk) {
+                        const int leader = __ffs(mk) - 1;
+                        unsigned base = 0;
+                        if (lane == leader) base = atomicAdd(a.recheck_count, (unsigned)__popc(mk));
+                        base = __shfl_sync(0xffffffffu, base, leader);
+                        if (push) a.recheck[base + __popc(mk & ((1u << lane) - 1u))] = (int)li;
+                    }
+                }
+                if (MODE == MODE_TICK && valid && !push) {               // a5: this candidate's key
                     const bool safe = steps == H;
                     float d2 = 0.f;
 #pragma unroll
@@ -472,7 +525,8 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         return;
     }
     // ---- a6 + a7
-    block_select_and_finalise<kTcStateWarps + 1>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, a.work);
+    block_select_and_finalise<kTcStateWarps + 1>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, a.work,
+                                                  (D == 32) && a.recheck != nullptr);
 }
 
 }  // namespace mpmi
