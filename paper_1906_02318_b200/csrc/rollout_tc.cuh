@@ -429,7 +429,6 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
 #pragma unroll
                     for (int j = 0; j < NB; j++) x[j] = __uint_as_float(hc == 0 ? r[j] : rp[j]);
                     alive = safe_check_par<NB>(cfg, x, nbox) && was_alive;
-                    if (verify) near = near || (was_alive && near_boundary<NB>(cfg, x, nbox, tau_box, tau_ann2));
                     steps += alive ? 1 : 0;
                 }
                 if (hc == 0) {
@@ -462,6 +461,12 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     fence_before_sync();
                     mbar_arrive(bar_alo);
                     SWT(sw_st);
+                }
+                if (verify && hc == 0) {                                 // off the step's critical path: after the hand-back
+                    float x[NB];
+#pragma unroll
+                    for (int j = 0; j < NB; j++) x[j] = __uint_as_float(r[j]);
+                    near = near || (was_alive && near_boundary<NB>(cfg, x, nbox, tau_box, tau_ann2));
                 }
             }
             if (dump && li < ncand) {                                    // states after the tile stopped: NaN
