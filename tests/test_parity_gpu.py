@@ -390,6 +390,39 @@ def test_tensor32_verified_tick(mp):
     assert worst <= TRAJ_RTOL, worst
 
 
+def test_tensor32_device_and_shard_paths(mp):
+    """The verified tensor-core tick through mpmi_step_device and as two candidate shards + finalize (both passes run per shard,
+    the FP32 pass writes the shard's partial): same result as the graph path and as the default FP32 tick."""
+    V = mp.mpmi
+    w = W.make("C4", N=(1 << 18) + 333)
+    ctx = mp.Context(w, variant=V.VARIANT_TENSOR32)
+    fp32 = mp.Context(w)
+    cut = (1 << 17) + 5
+    sh = [mp.Context(w, shard=(0, cut), variant=V.VARIANT_TENSOR32), mp.Context(w, shard=(cut, w.N + 1 - cut), variant=V.VARIANT_TENSOR32)]
+    assert ctx.info()["variant"] == 4 and all(c.info()["variant"] == 4 and c.info()["launches_per_tick"] == 4 for c in sh)
+    x0s, uus, ticks = W.tick_inputs(w, 5)
+    d_res = torch.zeros(56, dtype=torch.uint8, device="cuda")
+    d_parts = torch.zeros(2 * 24, dtype=torch.uint8, device="cuda")
+    s = torch.cuda.current_stream().cuda_stream
+    for x0, uu, t in zip(x0s, uus, ticks):
+        host = ctx.step_sync(x0, uu, int(t)).as_dict(w.m)
+        f = fp32.step_sync(x0, uu, int(t)).as_dict(w.m)
+        assert (host["index"], host["safe"], host["steps"], host["n_safe"], host["n_exec"]) == (f["index"], f["safe"], f["steps"], f["n_safe"], f["n_exec"])
+        dx, du = _dev(x0), _dev(uu)
+        ctx.step_device(dx.data_ptr(), du.data_ptr(), int(t), s, d_res.data_ptr())
+        torch.cuda.synchronize()
+        dev = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=V.RESULT_DTYPE)[0]
+        for g in range(2):
+            sh[g].shard_step(dx.data_ptr(), du.data_ptr(), int(t), s, d_parts.data_ptr() + 24 * g)
+        sh[0].shard_finalize(d_parts.data_ptr(), 2, du.data_ptr(), int(t), s, d_res.data_ptr())
+        torch.cuda.synchronize()
+        shd = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=V.RESULT_DTYPE)[0]
+        for got in (dev, shd):
+            assert got["index"] == host["index"] and got["safe"] == host["safe"] and got["steps"] == host["steps"]
+            assert got["n_safe"] == host["n_safe"] and got["n_exec"] == host["n_exec"] and got["key"] == host["key"]
+            assert np.array_equal(got["u"][: w.m], host["u"]) and got["dist"] == host["dist"]
+
+
 def test_edge_cases(mp):
     w = W.make("C1", N=1)
     o = _oracle(w)
