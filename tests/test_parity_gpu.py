@@ -373,6 +373,14 @@ def test_tensor32_verified_tick(mp):
             r = a.step_sync(x0, uu, int(t)).as_dict(w.m); f = b.step_sync(x0, uu, int(t)).as_dict(w.m)
             assert r["safe"] == branch
             assert (r["index"], r["safe"], r["steps"], r["n_safe"], r["n_exec"]) == (f["index"], f["safe"], f["steps"], f["n_safe"], f["n_exec"])
+    # with prediction noise (Alg. 2 l.5): both passes draw the same Philox normals; same result as the FP32 noise tick
+    wn = W.make("C4", N=N); wn.noise_sigma = 0.01
+    a, b = mp.Context(wn, variant=V.VARIANT_TENSOR32), mp.Context(wn)
+    assert a.info()["variant"] == 4 and a.info()["launches_per_tick"] == 4 and b.info()["variant"] == 1
+    for x0, uu, t in zip(x0s[:6], uus[:6], ticks[:6]):
+        r = a.step_sync(x0, uu, int(t)).as_dict(w.m); f = b.step_sync(x0, uu, int(t)).as_dict(w.m)
+        assert (r["index"], r["safe"], r["steps"], r["n_safe"], r["n_exec"]) == (f["index"], f["safe"], f["steps"], f["n_safe"], f["n_exec"]), (r, f)
+    del a, b
     # batch entry: FP32 register kernels, T1 + T2
     n1 = 1536 + 77
     rng = np.random.default_rng(5)
