@@ -72,7 +72,7 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
        MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32, >= 2^17 candidates: VERIFIED tensor-core tick.  The
                                            3xTF32 tcgen05 kernel (N = 32 MMAs, four CTAs per SM) rolls all
                                            candidates; every candidate whose state came within tau of the
-                                           safe-set boundary (tau ~ 6e-5 x the bounds, ~5 x the worst
+                                           safe-set boundary (tau ~ 1.25e-4 x the bounds, 5-6 x the worst
                                            3xTF32-vs-FP32 state difference) is rolled again by the FP32
                                            register kernel, which merges its keys and finalises: flags and
                                            winner are those of the FP32 tick.  mpmi_rollout_batch of such a

@@ -29,6 +29,7 @@ struct KArgs {
     int *recheck;                         // device, capacity = local candidates, or null
     unsigned *recheck_count;              // device; zeroed by the CTA that finalises
     int recheck_mode;                     // register kernel: 1 = walk recheck[0 .. *recheck_count) instead of the index space
+    float recheck_tau_scale;              // scales tau (1 = the built-in threshold; the safety-factor measurement sets it < 1)
     // batch
     const float *U;                       // device Ncand*m or null
     long long x0_count;

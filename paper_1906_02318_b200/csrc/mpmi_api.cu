@@ -6,6 +6,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -69,6 +70,7 @@ struct mpmi_ctx {
     int *d_recheck = nullptr;
     unsigned *d_recheck_count = nullptr;
     unsigned recheck_grid = 0;
+    float recheck_tau_scale = 1.f;   // MPMI_TC32_TAU_SCALE (measurement of the threshold's safety factor only)
     cudaGraphNode_t n_recheck = nullptr;
     KArgs gr{};
     std::string err;
@@ -240,7 +242,7 @@ void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
     if (c->affine) launch_base(c, a, s);
-    if (c->k_recheck) { a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; }
+    if (c->k_recheck) { a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale; }
     launch(c, c->k_tick, c->dc.shard_count, a, s);
     if (c->k_recheck) {                          // second pass: FP32 register kernel over the deferred candidates
         a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1; a.kslot = c->kslot; a.work = nullptr;
@@ -291,7 +293,7 @@ void recheck_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
 int build_graph(mpmi_ctx *c) {
     c->ga = KArgs{};
     c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1; c->ga.kslot = c->kslot;
-    if (c->k_recheck) { c->ga.recheck = c->d_recheck; c->ga.recheck_count = c->d_recheck_count; }
+    if (c->k_recheck) { c->ga.recheck = c->d_recheck; c->ga.recheck_count = c->d_recheck_count; c->ga.recheck_tau_scale = c->recheck_tau_scale; }
     if (c->variant == 2 || c->variant == 4) c->ga.work = &c->d_state->work;
     c->tick_grid = grid_for(c, c->dc.shard_count);
     CU(c, cudaGraphCreate(&c->graph, 0));
@@ -604,6 +606,10 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc));
             CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned)));
             CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned)));
+            if (const char *e = std::getenv("MPMI_TC32_TAU_SCALE")) {
+                const float v = (float)std::atof(e);
+                if (v > 0.f && v <= 16.f) c->recheck_tau_scale = v;
+            }
         }
     } else {
         // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)

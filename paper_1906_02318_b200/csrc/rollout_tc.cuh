@@ -319,18 +319,20 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
         const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
         const float qnan = __int_as_float(0x7fc00000);
-        // verified tick: tau = 6e-5 x the size of the bounds (>= 5e-4).  Measured on C4 (|x| ~ 10, |z| ~ 130): the 3xTF32
-        // states drift from the FP32 ones by <= 1.5e-5 relative over H = 100 steps (flags differ from the oracle's only at
-        // margins <= 1.4e-4), so tau = 7.2e-4 there is ~5x the worst difference; ~3 % of the candidates take the second pass
+        // verified tick: tau = 1.25e-4 x the size of the bounds (>= 1e-3).  Measured on C4 (|x| ~ 10, |z| ~ 130, bounds 12) with
+        // MPMI_TC32_TAU_SCALE over 40 ticks x 2^20 candidates: the result equals the FP32 tick's down to tau = 2.9e-4 and
+        // first differs at 2.5e-4 (the largest 3xTF32-vs-FP32 state difference that decides a flag), so tau = 1.5e-3 there is
+        // 5-6x that; ~6.5 % of the candidates take the second pass
         const bool verify = (D == 32) && (MODE == MODE_TICK) && a.recheck != nullptr;
-        float tau_box = 5e-4f, tau_ann2 = 0.f;
+        float tau_box = 1e-3f, tau_ann2 = 0.f;
         if (verify) {
             for (int j = 0; j < nbox && j < NB; j++) {
-                if (isfinite(cfg.blo[j])) tau_box = fmaxf(tau_box, 6e-5f * fabsf(cfg.blo[j]));
-                if (isfinite(cfg.bhi[j])) tau_box = fmaxf(tau_box, 6e-5f * fabsf(cfg.bhi[j]));
+                if (isfinite(cfg.blo[j])) tau_box = fmaxf(tau_box, 1.25e-4f * fabsf(cfg.blo[j]));
+                if (isfinite(cfg.bhi[j])) tau_box = fmaxf(tau_box, 1.25e-4f * fabsf(cfg.bhi[j]));
             }
             const float rmax = sqrtf(cfg.rmax2);
-            tau_ann2 = 2.f * rmax * fmaxf(5e-4f, 6e-5f * rmax);
+            tau_box *= a.recheck_tau_scale;
+            tau_ann2 = 2.f * rmax * fmaxf(1e-3f, 1.25e-4f * rmax) * a.recheck_tau_scale;
         }
         unsigned p_full = 0, p_tile = 0;
 #ifdef MPMI_TC_DEBUG
