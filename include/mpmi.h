@@ -76,7 +76,9 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
                                            3xTF32-vs-FP32 state difference) is rolled again by the FP32
                                            register kernel, which merges its keys and finalises: flags and
                                            winner are those of the FP32 tick.  mpmi_rollout_batch of such a
-                                           context runs the FP32 kernels             */
+                                           context runs the FP32 kernels.  The
+                                           environment variable MPMI_TC32_TAU_SCALE (0 < v <= 16, read by
+                                           mpmi_create) scales tau: a measurement aid, not a tuning knob     */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:
