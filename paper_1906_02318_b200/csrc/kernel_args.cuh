@@ -5,6 +5,7 @@
 namespace mpmi {
 
 constexpr int kRegBlock = 128;
+constexpr int kRecheckBuckets = 4;          // verified tensor-core tick: deferred candidates are listed per quarter of the horizon they survived
 
 struct KArgs {
     // tick
@@ -26,9 +27,9 @@ struct KArgs {
     // verified tensor-core tick (D = 32): candidates that came within tau of the safe-set boundary in the 3xTF32 rollout are
     // not keyed there but appended to `recheck`; the FP32 register kernel (recheck_mode = 1) rolls exactly those again,
     // merges its keys into the same TickState and finalises the tick
-    int *recheck;                         // device, capacity = local candidates, or null
-    unsigned *recheck_count;              // device; zeroed by the CTA that finalises
-    int recheck_mode;                     // register kernel: 1 = walk recheck[0 .. *recheck_count) instead of the index space
+    int *recheck;                         // device, kRecheckBuckets lists of capacity = local candidates each, or null
+    unsigned *recheck_count;              // device, one per list; zeroed by the CTA that finalises
+    int recheck_mode;                     // register kernel: 1 = walk the recheck lists (longest-lived first) instead of the index space
     float recheck_tau_scale;              // scales tau (1 = the built-in threshold; the safety-factor measurement sets it < 1)
     // batch
     const float *U;                       // device Ncand*m or null

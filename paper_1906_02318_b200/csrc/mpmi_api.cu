@@ -603,9 +603,9 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             // the second pass sees a few 10^4 candidates: below ~2^19 the shared-memory model is the faster one (section 9 sweep)
             c->k_recheck = pick_reg(D, M, 1, MODE_TICK, noise, 0);
             c->recheck_grid = (unsigned)((sc + 2 * kRegBlock - 1) / (2 * kRegBlock));
-            CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc));
-            CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned)));
-            CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned)));
+            CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc * kRecheckBuckets));
+            CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned) * kRecheckBuckets));
+            CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned) * kRecheckBuckets));
             if (const char *e = std::getenv("MPMI_TC32_TAU_SCALE")) {
                 const float v = (float)std::atof(e);
                 if (v > 0.f && v <= 16.f) c->recheck_tau_scale = v;

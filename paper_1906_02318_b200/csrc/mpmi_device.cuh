@@ -242,7 +242,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                                                           unsigned n_safe, unsigned long long n_exec,
                                                           unsigned long long tick, const float (&u_h)[kMaxM],
                                                           TickState *st, mpmi_result *out, mpmi_partial *partial,
-                                                          unsigned seq = 0, unsigned *work = nullptr, bool defer = false) {
+                                                          unsigned seq = 0, unsigned *work = nullptr, bool defer = false, int nwork = 1) {
     __shared__ unsigned long long s_key[kWarps];
     __shared__ unsigned s_safe[kWarps];
     __shared__ unsigned long long s_exec[kWarps];
@@ -282,7 +282,11 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                 decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out, seq);
             }
             st->best_key = kKeyNone; st->n_exec = 0ull; st->n_safe = 0u; st->ticket = 0u;   // ready for next tick
-            if (work) { st->pad = *work; *work = 0u; }
+            if (work) {
+                unsigned tot = 0;
+                for (int i = 0; i < nwork; i++) { tot += work[i]; work[i] = 0u; }
+                st->pad = tot;
+            }
             __threadfence();
         }
     }

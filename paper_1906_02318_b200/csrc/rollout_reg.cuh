@@ -69,8 +69,16 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         // the two halves of a register pair are ADJACENT candidates (2*tid, 2*tid+1): dumps store float2
         li[s] = (long long)blockIdx.x * (S * bdim) + (s >> 1) * (2 * bdim) + 2 * tid + (s & 1);
         if (MODE == MODE_TICK && a.perm && li[s] < a.nsamp) li[s] = a.perm[li[s]];   // spatially ordered walk
-        if (MODE == MODE_TICK && a.recheck_mode)                                      // second pass of the verified tensor-core tick
-            li[s] = li[s] < (long long)*a.recheck_count ? (long long)a.recheck[li[s]] : ncand;
+        if (MODE == MODE_TICK && a.recheck_mode) {                                    // second pass of the verified tensor-core tick
+            long long p = li[s], hit = ncand;                                         // slot p of the concatenated lists
+#pragma unroll
+            for (int b = 0; b < kRecheckBuckets; b++) {
+                const long long cb = (long long)a.recheck_count[b];
+                if (p >= 0 && p < cb) hit = (long long)a.recheck[(long long)b * ncand + p];
+                p -= cb;                                                              // negative once the slot has been found
+            }
+            li[s] = hit;
+        }
         const bool valid = li[s] < ncand && inputs_ok;
         alive[s] = valid;
         steps[s] = 0;
@@ -278,7 +286,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         }
     }
     block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq,
-                                              (MODE == MODE_TICK && a.recheck_mode) ? a.recheck_count : nullptr);
+                                              (MODE == MODE_TICK && a.recheck_mode) ? a.recheck_count : nullptr, false, kRecheckBuckets);
 }
 
 }  // namespace mpmi

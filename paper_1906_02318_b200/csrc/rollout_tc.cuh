@@ -489,13 +489,19 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 bool push = false;
                 if (MODE == MODE_TICK && verify) {                       // near the boundary: the FP32 kernel decides (warp-aggregated append)
                     push = valid && near;
-                    const unsigned mk = __ballot_sync(0xffffffffu, push);
-                    if (mk) {
-                        const int leader = __ffs(mk) - 1;
-                        unsigned base = 0;
-                        if (lane == leader) base = atomicAdd(a.recheck_count, (unsigned)__popc(mk));
-                        base = __shfl_sync(0xffffffffu, base, leader);
-                        if (push) a.recheck[base + __popc(mk & ((1u << lane) - 1u))] = (int)li;
+                    // kRecheckBuckets lists by the first pass's step count, longest first: the second pass then walks candidates
+                    // of similar life time together (its warps stop together, its long CTAs start first)
+                    const int bucket = kRecheckBuckets - 1 - min(kRecheckBuckets - 1, steps * kRecheckBuckets / H);
+#pragma unroll
+                    for (int b = 0; b < kRecheckBuckets; b++) {
+                        const unsigned mk = __ballot_sync(0xffffffffu, push && bucket == b);
+                        if (mk) {
+                            const int leader = __ffs(mk) - 1;
+                            unsigned base = 0;
+                            if (lane == leader) base = atomicAdd(a.recheck_count + b, (unsigned)__popc(mk));
+                            base = __shfl_sync(0xffffffffu, base, leader);
+                            if (push && bucket == b) a.recheck[(long long)b * ncand + base + __popc(mk & ((1u << lane) - 1u))] = (int)li;
+                        }
                     }
                 }
                 if (MODE == MODE_TICK && valid && !push) {               // a5: this candidate's key
