@@ -69,6 +69,9 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
                                            sample-step; ignored with noise or the re-lift model   */
        MPMI_VARIANT_NO_PREDICT = 512,   /* d > 32: walk the candidates in input-box-cell order instead of
                                            the order of their predicted life time                 */
+       MPMI_VARIANT_SMEM_MODEL = 2048,  /* d <= 32: model staged in shared memory (LDS.128) even where the constant
+                                           bank would be chosen -- the variant a context falls back to when all
+                                           constant-memory slots of its device are taken                      */
        MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32, >= 2^17 candidates: VERIFIED tensor-core tick.  The
                                            3xTF32 tcgen05 kernel (N = 32 MMAs, four CTAs per SM) rolls all
                                            candidates; every candidate whose state came within tau of the
@@ -95,7 +98,9 @@ typedef struct {
 /* Safe set: AND of
  *   box constraints   lo[q] + inflate <  x[idx[q]]  <  hi[q] - inflate   (strict; +-INFINITY allowed)
  *   optional annulus  rmin + inflate <= hypot(x[ix]-cx, x[iy]-cy) <= rmax - inflate   (closed)
- * NaN / Inf states are unsafe.  inflate is the hand-tuned inflation radius of PAPER.md:221. */
+ * Only constrained dims (box idx, annulus ix / iy) are tested: NaN or Inf there is unsafe, an unconstrained
+ * physical dim is never looked at (same rule in every kernel and in the oracle).
+ * inflate is the hand-tuned inflation radius of PAPER.md:221. */
 typedef struct {
     int32_t        nbounds;
     const int32_t *idx;       /* host, nbounds, each < n              */
@@ -192,6 +197,15 @@ int mpmi_step_sync(mpmi_ctx *ctx, const float *x0, const float *u_user, uint64_t
  * inputs give a result with index = -1. */
 int mpmi_step_device(mpmi_ctx *ctx, const float *d_x0, const float *d_u_user, uint64_t tick,
                      void *cuda_stream, mpmi_result *d_out);
+
+/* Diagnostic twin of mpmi_step_device: the SAME kernels in the SAME launch configuration (binning, tensor-core first
+ * pass + FP32 second pass, ...), which additionally store the step count of every local candidate as the tick kernels
+ * decided it: d_steps (device, ncand_local int32; entry = global candidate index - shard_begin; the injected user
+ * input is the last entry of the shard that owns index N) = safe predicted states before the first violation
+ * (H <=> safe).  This is what the full-size parity tests compare with the oracle candidate by
+ * candidate; the extra 4-byte store per candidate is the only difference to mpmi_step_device.  Asynchronous. */
+int mpmi_step_trace(mpmi_ctx *ctx, const float *d_x0, const float *d_u_user, uint64_t tick,
+                    void *cuda_stream, mpmi_result *d_out, int32_t *d_steps);
 
 /* Sharded tick (section 8(e)): roll out this context's shard and write its mpmi_partial to
  * d_partial (device).  After the caller has gathered the G partials of all ranks into d_partials

@@ -1,7 +1,8 @@
 """Calibration of the synthetic workloads (SURVEY.md 8(d) protocol) -- calls ONLY oracle/ and
 workloads/.  Writes workloads/calibration.json, which workloads.generate.make() reads.
 
-  python -m oracle.calibrate
+  python -m oracle.calibrate              # C1..C5 (BASELINE.json configs) and the extra test workloads
+  python -m oracle.calibrate T48 T4       # only these, merged into the existing file
 
 For each config: (1) advance the model seed until the zero-input rollout from x_nom is safe over
 H; (2) bisect the input gain gamma in [1e-3, 1e3] (geometric, 40 iterations) until the oracle's
@@ -14,7 +15,7 @@ from oracle.oracle import Oracle
 from workloads import generate as G
 
 TARGET, TOL = 0.40, 0.02
-N_CAL = {"C1": 1024, "C2": 10000, "C3": 10000, "C4": 16384, "C5": 4096}
+N_CAL = {"C1": 1024, "C2": 10000, "C3": 10000, "C4": 16384, "C5": 4096, "T48": 4096, "T4": 4096}
 
 
 def safe_fraction(w, N):
@@ -60,8 +61,10 @@ def calibrate(name):
 
 
 def main():
-    cal = {}
-    for name in G.CONFIG_NAMES:
+    import sys
+    names = sys.argv[1:] or list(G.CONFIG_NAMES + G.TEST_NAMES)
+    cal = G.load_calibration() if sys.argv[1:] else {}
+    for name in names:
         if name == "C4":                       # same model as C3 (BASELINE.json configs[3])
             cal["C4"] = dict(cal["C3"])
         else:

@@ -4,6 +4,7 @@
 // pinned staging, and the benchmark entry mpmi_rollout_batch.  No CPU fallback: every step of the
 // path runs in the kernels of rollout_reg.cuh / rollout_tile.cuh.
 #include <atomic>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -11,7 +12,11 @@
 #include <mutex>
 #include <new>
 #include <string>
+#include <thread>
 #include <vector>
+#if defined(__x86_64__) || defined(__i386__)
+#include <immintrin.h>
+#endif
 #include <cuda_runtime.h>
 #include "../../include/mpmi.h"
 #include "mpmi_device.cuh"
@@ -100,6 +105,14 @@ constexpr long long kTc32MinCand = 1LL << 17;   // D = 32: tensor-core kernel fr
 
 thread_local std::string g_create_err;
 
+inline void cpu_relax() {
+#if defined(__x86_64__) || defined(__i386__)
+    _mm_pause();
+#elif defined(__aarch64__)
+    asm volatile("yield" ::: "memory");
+#endif
+}
+
 #define CU(ctx, call)                                                                      \
     do {                                                                                   \
         cudaError_t e_ = (call);                                                           \
@@ -147,17 +160,20 @@ KernFn pick_reg(int D, int M, int P, int mode, bool noise, int kconst = 1) {
     return nullptr;
 }
 // constant-memory model slots of the register kernels: one per live context (kernel_args.cuh: kModelSlots)
+// (__constant__ memory is per device, so is the slot table: 8 live register-kernel contexts per GPU)
+constexpr int kMaxDevices = 64;
 std::mutex g_slot_mu;
-bool g_slot_used[kModelSlots] = {};
-int slot_acquire() {
+bool g_slot_used[kMaxDevices][kModelSlots] = {};
+int slot_acquire(int dev) {
+    if (dev < 0 || dev >= kMaxDevices) return -1;
     std::lock_guard<std::mutex> lk(g_slot_mu);
-    for (int i = 0; i < kModelSlots; i++) if (!g_slot_used[i]) { g_slot_used[i] = true; return i; }
+    for (int i = 0; i < kModelSlots; i++) if (!g_slot_used[dev][i]) { g_slot_used[dev][i] = true; return i; }
     return -1;
 }
-void slot_release(int i) {
-    if (i < 0) return;
+void slot_release(int dev, int i) {
+    if (i < 0 || dev < 0 || dev >= kMaxDevices) return;
     std::lock_guard<std::mutex> lk(g_slot_mu);
-    g_slot_used[i] = false;
+    g_slot_used[dev][i] = false;
 }
 // the slot is filled in the translation units of the tick and batch kernels this context launches
 int set_model(int D, bool noise, int slot, const float *kta, int nfloats) {
@@ -189,8 +205,9 @@ bool all_finite(const float *p, size_t n) {
     return true;
 }
 
-void launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s, int cpb, int block, int smem,
-                 bool persistent) {
+// every launch returns its status: the callers hand it to CU() (no launch result is dropped)
+cudaError_t launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s, int cpb, int block, int smem,
+                        bool persistent) {
     long long blocks = (ncand + cpb - 1) / cpb;
     if (blocks < 1) blocks = 1;
     KArgs a = a0;
@@ -200,19 +217,18 @@ void launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0,
     }
     a.kslot = c->kslot;
     void *args[2] = {(void *)&c->dc, (void *)&a};
-    cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)smem, s);
+    return cudaLaunchKernel((const void *)fn, dim3((unsigned)blocks), dim3((unsigned)block), args, (size_t)smem, s);
 }
-void launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
+cudaError_t launch(const mpmi_ctx *c, KernFn fn, long long ncand, const KArgs &a0, cudaStream_t s) {
     if (fn == c->k_batch_aff && fn != nullptr)
-        launch_geom(c, fn, ncand, a0, s, 256, 256, a0.H * (1 + c->dc.m) * c->dc.aff_np * 4, false);
-    else if (fn == c->k_batch)
-        launch_geom(c, fn, ncand, a0, s, c->bcand_per_block, c->bblock, c->bsmem, c->bpersistent);
-    else
-        launch_geom(c, fn, ncand, a0, s, c->cand_per_block, c->block, c->smem, c->variant == 2 || c->variant == 4);
+        return launch_geom(c, fn, ncand, a0, s, 256, 256, a0.H * (1 + c->dc.m) * c->dc.aff_np * 4, false);
+    if (fn == c->k_batch)
+        return launch_geom(c, fn, ncand, a0, s, c->bcand_per_block, c->bblock, c->bsmem, c->bpersistent);
+    return launch_geom(c, fn, ncand, a0, s, c->cand_per_block, c->block, c->smem, c->variant == 2 || c->variant == 4);
 }
-void launch_base(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {      // a_k = C K^k Psi(x_t) of the affine path
+cudaError_t launch_base(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {      // a_k = C K^k Psi(x_t) of the affine path
     void *args[2] = {(void *)&c->dc, (void *)&a};
-    cudaLaunchKernel((const void *)c->k_base, dim3((unsigned)c->dc.H), dim3(128), args, 0, s);
+    return cudaLaunchKernel((const void *)c->k_base, dim3((unsigned)c->dc.H), dim3(128), args, 0, s);
 }
 
 // one tick on stream s: [cell histogram + scan, scatter] (large Philox sets only) -> fused tick kernel
@@ -224,32 +240,35 @@ const void *pick_predict_m(int m) {
 const void *pick_predict(int np, int m) { return np == 4 ? pick_predict_m<4>(m) : np == 8 ? pick_predict_m<8>(m) : pick_predict_m<16>(m); }
 unsigned pred_smem(const mpmi_ctx *c) { return (unsigned)(c->dc.H * (1 + c->dc.m) * c->dc.aff_np * 4); }
 
-void enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
+#define CL(call) do { const cudaError_t e_ = (call); if (e_ != cudaSuccess) return e_; } while (0)
+cudaError_t enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
     if (c->binning) {
         BinArgs b = c->bin;
         b.tick_val = a.tick_val;
         long long g = (b.nsamp + 255) / 256;
         const long long gmax = 8LL * c->sm_count;
         const unsigned grid = (unsigned)(g < gmax ? g : gmax);
+        void *pargs[2] = {(void *)&c->dc, (void *)&b};
         if (c->predict) {        // a_k for this x_t, then predicted life times (keys) + their histogram + scan
-            launch_base(c, a, s);
-            void *pargs[2] = {(void *)&c->dc, (void *)&b};
-            cudaLaunchKernel(c->k_pred, dim3((unsigned)g), dim3(256), pargs, pred_smem(c), s);
+            CL(launch_base(c, a, s));
+            CL(cudaLaunchKernel(c->k_pred, dim3((unsigned)g), dim3(256), pargs, pred_smem(c), s));
         } else {
-            bin_hist_kernel<<<grid, 256, 0, s>>>(c->dc, b);
+            CL(cudaLaunchKernel((const void *)bin_hist_kernel, dim3(grid), dim3(256), pargs, 0, s));
         }
-        bin_scatter_kernel<<<grid, 256, 0, s>>>(c->dc, b);
+        CL(cudaLaunchKernel((const void *)bin_scatter_kernel, dim3(grid), dim3(256), pargs, 0, s));
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
-    if (c->affine) launch_base(c, a, s);
+    if (c->affine) CL(launch_base(c, a, s));
     if (c->k_recheck) { a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale; }
-    launch(c, c->k_tick, c->dc.shard_count, a, s);
+    CL(launch(c, c->k_tick, c->dc.shard_count, a, s));
     if (c->k_recheck) {                          // second pass: FP32 register kernel over the deferred candidates
         a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1; a.kslot = c->kslot; a.work = nullptr;
         void *args[2] = {(void *)&c->dc, (void *)&a};
-        cudaLaunchKernel((const void *)c->k_recheck, dim3(c->recheck_grid), dim3(kRegBlock), args, 0, s);
+        CL(cudaLaunchKernel((const void *)c->k_recheck, dim3(c->recheck_grid), dim3(kRegBlock), args, 0, s));
     }
+    return cudaSuccess;
 }
+#undef CL
 
 unsigned grid_for(const mpmi_ctx *c, long long ncand) {
     long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
@@ -360,7 +379,7 @@ void mpmi_destroy(mpmi_ctx *c) {
     if (c->graph) cudaGraphDestroy(c->graph);
     cudaFree(c->d_affM); cudaFree(c->d_KTa); cudaFree(c->d_W); cudaFree(c->d_b); cudaFree(c->d_terms);
     cudaFree(c->d_state);
-    slot_release(c->kslot);
+    slot_release(c->device, c->kslot);
     cudaFree(c->d_affA); cudaFree(c->d_affG);
     cudaFree(c->d_pred);
     cudaFree(c->d_recheck); cudaFree(c->d_recheck_count);
@@ -558,9 +577,9 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         // model source: the constant bank (one slot per context) when the grid fills the machine or the model fits the
         // immediate constant cache, shared memory otherwise (measured crossover at D = 32: ~2^19 candidates); the batch
         // kernels take the constant bank whenever a slot is free (it frees the LSU for the trajectory stores)
-        c->kslot = slot_acquire();
+        c->kslot = (cfg->variant & MPMI_VARIANT_SMEM_MODEL) ? -1 : slot_acquire(dev);
         if (c->kslot >= 0 && set_model(D, noise, c->kslot, KTa.data(), (int)KTa.size()) != 0) {
-            slot_release(c->kslot); c->kslot = -1; (void)cudaGetLastError();
+            slot_release(dev, c->kslot); c->kslot = -1; (void)cudaGetLastError();
         }
         const int kconst_tick = (c->kslot >= 0 && ((D + M) * D * 4 <= 2048 || sc >= (1LL << 19))) ? 1 : 0;
         const int kconst_batch = c->kslot >= 0 ? 1 : 0;
@@ -590,7 +609,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         // D = 32, large candidate sets, on request (MPMI_VARIANT_TENSOR32: its flags are not within the 1e-4 margin rule at
         // large state magnitudes): the same 3xTF32 tcgen05 kernel as at d = 128, with N = 32 MMAs and four CTAs per SM
         if (D == 32 && c->variant == 1 && (cfg->variant & MPMI_VARIANT_TENSOR32) && sc >= kTc32MinCand && (!noise || n <= 8) &&
-            !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY))) {
+            !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY | MPMI_VARIANT_AFFINE))) {
             // The tick is VERIFIED: candidates whose 3xTF32 state came near the safe-set boundary are rolled again by the
             // FP32 register kernel (2 candidates per thread), so flags and winner are those of the FP32 path.  The batch
             // entry stays on the FP32 register kernels chosen above.
@@ -777,12 +796,19 @@ int mpmi_step_result(mpmi_ctx *c, mpmi_result *out) {
     // number; poll for it (cheaper than a stream synchronise), checking the stream for errors now and then
     volatile mpmi_result *h = c->h_res;
     const int want = (int)c->seq;
+    // back-off: a tight poll (with the CPU's spin-wait hint) for the first ~2^14 reads -- a paper-scale tick takes tens of
+    // microseconds and the poll is what the latency harness times -- then the core is yielded between reads, and past ~2^20
+    // reads (a tick that takes seconds: debugger, sanitizer, a time-sliced GPU) the thread sleeps 50 us per read
     for (unsigned spin = 0; h->reserved != want; spin++) {
-        if ((spin & 0x3FFF) == 0x3FFF) {
+        if ((spin & 0x3FFF) == 0x3FFF || spin >= (1u << 20)) {
+            if (spin == 0xFFFFFFFFu) spin = 1u << 20;
             const cudaError_t e = cudaStreamQuery(c->pending_stream);
             if (e == cudaSuccess) { if (h->reserved != want) { c->pending = false; return fail(c, MPMI_ERR_CUDA, "tick finished without a result"); } break; }
             if (e != cudaErrorNotReady) { c->pending = false; c->err = std::string("tick failed: ") + cudaGetErrorString(e); return MPMI_ERR_CUDA; }
         }
+        if (spin < (1u << 14)) cpu_relax();
+        else if (spin < (1u << 20)) std::this_thread::yield();
+        else std::this_thread::sleep_for(std::chrono::microseconds(50));
     }
     std::atomic_thread_fence(std::memory_order_acquire);
     c->pending = false;
@@ -804,8 +830,18 @@ int mpmi_step_device(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint
     KArgs a{};
     a.x0 = d_x0; a.u_user = d_u_user; a.tick_val = tick;
     a.st = c->d_state; a.out = d_out;
-    enqueue_tick(c, a, (cudaStream_t)stream);
-    CU(c, cudaGetLastError());
+    CU(c, enqueue_tick(c, a, (cudaStream_t)stream));
+    return MPMI_OK;
+}
+
+int mpmi_step_trace(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint64_t tick, void *stream, mpmi_result *d_out, int32_t *d_steps) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (!d_x0 || !d_u_user || !d_out || !d_steps) return fail(c, MPMI_ERR_INVALID, "null device pointer");
+    CU(c, cudaSetDevice(c->device));
+    KArgs a{};
+    a.x0 = d_x0; a.u_user = d_u_user; a.tick_val = tick;
+    a.st = c->d_state; a.out = d_out; a.steps = d_steps;
+    CU(c, enqueue_tick(c, a, (cudaStream_t)stream));
     return MPMI_OK;
 }
 
@@ -816,8 +852,7 @@ int mpmi_shard_step(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint6
     KArgs a{};
     a.x0 = d_x0; a.u_user = d_u_user; a.tick_val = tick;
     a.st = c->d_state; a.out = nullptr; a.partial = d_partial;
-    enqueue_tick(c, a, (cudaStream_t)stream);
-    CU(c, cudaGetLastError());
+    CU(c, enqueue_tick(c, a, (cudaStream_t)stream));
     return MPMI_OK;
 }
 
@@ -845,14 +880,13 @@ int mpmi_rollout_batch(mpmi_ctx *c, const float *d_U, const float *d_X0, int64_t
     a.U = d_U; a.x0_count = x0_count; a.ncand = Ncand; a.H = H; a.dump_kind = dump_kind;
     a.traj = d_traj; a.steps = d_steps; a.safe = d_safe;
     if (c->affine && dump_kind != MPMI_DUMP_LIFTED && x0_count == 1 && H <= c->dc.H) {
-        launch_base(c, a, (cudaStream_t)stream);                 // physical states only, shared x0: the affine path applies
-        launch(c, c->k_batch_aff, Ncand, a, (cudaStream_t)stream);
+        CU(c, launch_base(c, a, (cudaStream_t)stream));          // physical states only, shared x0: the affine path applies
+        CU(c, launch(c, c->k_batch_aff, Ncand, a, (cudaStream_t)stream));
     } else if (dump_kind != MPMI_DUMP_NONE && c->k_batch_dump && c->variant != 5) {
-        launch_geom(c, c->k_batch_dump, Ncand, a, (cudaStream_t)stream, 256, 128, 0, false);
+        CU(c, launch_geom(c, c->k_batch_dump, Ncand, a, (cudaStream_t)stream, 256, 128, 0, false));
     } else {
-        launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream);
+        CU(c, launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream));
     }
-    CU(c, cudaGetLastError());
     return MPMI_OK;
 }
 

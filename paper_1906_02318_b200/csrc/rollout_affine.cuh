@@ -124,6 +124,7 @@ __global__ void __launch_bounds__(kAffBlock) rollout_affine_kernel(const __grid_
     }
     unsigned long long key = kKeyNone;
     unsigned n_safe = 0, n_exec = 0;
+    if (a.steps && li < ncand) a.steps[li] = steps;             // mpmi_step_trace: per-candidate steps of THIS tick kernel
     if (valid) {
         const bool safe = steps == H;
         float d2 = 0.f;

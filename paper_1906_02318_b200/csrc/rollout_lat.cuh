@@ -61,6 +61,11 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     }
     const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
     const bool no_annulus = cfg.annulus == 0;
+    // only constrained dims are tested (as in every other kernel and in the oracle): an unconstrained dim passes whatever
+    // it holds, Inf and NaN included -- its (-inf, +inf) limits alone would reject those
+    bool unc[NB];
+#pragma unroll
+    for (int j = 0; j < NB; j++) unc[j] = ((cfg.bmask >> j) & 1u) == 0u;
 
     // ---- a3 + a4: no memory traffic inside this loop -----------------------------------------------
     for (int k = 0; k < H; k++) {
@@ -84,11 +89,11 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
             for (int r = 0; r < R; r++)
                 z[qq * R + r] = __shfl_sync(0xffffffffu, (r & 1) ? acc[r / 2].y : acc[r / 2].x, qq, L);
 
-        // a4, branch-free for the common shapes: dims 0..3 against their limits (+-inf where there is
+        // a4, branch-free for the common shapes: dims 0..3 against their limits (always true where there is
         // none), the annulus folded in arithmetically; only more than 4 boxed dims take a branch
         bool ok = true;
 #pragma unroll
-        for (int j = 0; j < 4 && j < NB; j++) ok = ok & (z[j] > cfg.blo[j]) & (z[j] < cfg.bhi[j]);
+        for (int j = 0; j < 4 && j < NB; j++) ok = ok & (((z[j] > cfg.blo[j]) & (z[j] < cfg.bhi[j])) | unc[j]);
         {
             const float dx = __fsub_rn(z[0], cfg.cx), dy = __fsub_rn(z[1], cfg.cy);
             const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
@@ -96,7 +101,7 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         }
         if (nbox > 4) {
 #pragma unroll
-            for (int j = 4; j < NB; j++) ok = ok & (z[j] > cfg.blo[j]) & (z[j] < cfg.bhi[j]);
+            for (int j = 4; j < NB; j++) ok = ok & (((z[j] > cfg.blo[j]) & (z[j] < cfg.bhi[j])) | unc[j]);
         }
         alive = alive & ok;
         steps += alive ? 1 : 0;
@@ -105,6 +110,7 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     // ---- a5-a7 ------------------------------------------------------------------------------------
     unsigned long long key = kKeyNone;
     unsigned n_safe = 0, n_exec = 0;
+    if (a.steps && q == 0 && li < ncand) a.steps[li] = steps;    // mpmi_step_trace
     if (q == 0 && li < ncand && inputs_ok) {
         const bool safe = steps == H;
         float d2 = 0.f;

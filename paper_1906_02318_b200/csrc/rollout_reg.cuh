@@ -270,6 +270,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     unsigned n_safe = 0, n_exec = 0;
 #pragma unroll
     for (int s = 0; s < S; s++) {
+        if (a.steps && li[s] < ncand) a.steps[li[s]] = steps[s];   // mpmi_step_trace: per-candidate steps of THIS tick kernel
         if (li[s] < ncand && inputs_ok) {
             const bool safe = steps[s] == H;
             float d2 = 0.f;

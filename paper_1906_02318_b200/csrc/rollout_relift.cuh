@@ -212,6 +212,7 @@ rollout_relift_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant_
     // ---- a5-a7: key, argmin, finalise
     unsigned long long key = kKeyNone;
     unsigned n_safe = 0, n_exec = 0;
+    if (a.steps && li < ncand) a.steps[li] = steps;             // mpmi_step_trace: per-candidate steps of THIS tick kernel
     if (valid) {
         const bool safe = steps == H;
         float d2 = 0.f;

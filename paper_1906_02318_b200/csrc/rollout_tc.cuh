@@ -504,6 +504,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                         }
                     }
                 }
+                if (MODE == MODE_TICK && a.steps && valid) a.steps[li] = steps;   // mpmi_step_trace (a deferred candidate: overwritten by the second pass)
                 if (MODE == MODE_TICK && valid && !push) {               // a5: this candidate's key
                     const bool safe = steps == H;
                     float d2 = 0.f;

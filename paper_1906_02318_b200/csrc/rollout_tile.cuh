@@ -201,6 +201,7 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
                 if (a.safe) a.safe[li] = steps == H ? 1 : 0;
             }
         } else if (li < ncand && inputs_ok && lane < WC) {  // a5: this candidate's key
+            if (a.steps) a.steps[li] = steps;               // mpmi_step_trace
             const bool safe = steps == H;
             float d2 = 0.f;
 #pragma unroll

@@ -28,16 +28,28 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
-// bounded wait: a protocol error traps instead of hanging the GPU
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// bounded wait: a protocol error traps instead of hanging the GPU.  The bound is WALL TIME (20 s on one barrier phase),
+// not a poll count: under a debugger, compute-sanitizer, MPS time-slicing or a preempted context a healthy kernel may
+// poll millions of times, and must not be killed for it.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    for (unsigned spin = 0; !mbar_try_wait(bar, parity); spin++)
-        if (spin > (1u << 22)) {
+    unsigned long long t0 = 0;
+    for (unsigned spin = 1; !mbar_try_wait(bar, parity); spin++)
+        if ((spin & 0xFFFFu) == 0u) {
+            const unsigned long long t = globaltimer_ns();
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > 20000000000ull) {
 #ifdef MPMI_TC_DEBUG
-            printf("mbar timeout: bar %x parity %u thread %d block %d\n", bar, parity, (int)threadIdx.x, (int)blockIdx.x);
-            return;
+                printf("mbar timeout: bar %x parity %u thread %d block %d\n", bar, parity, (int)threadIdx.x, (int)blockIdx.x);
+                return;
 #else
-            __trap();
+                __trap();
 #endif
+            }
         }
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }

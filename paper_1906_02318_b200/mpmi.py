@@ -16,10 +16,10 @@ DUMP_NONE, DUMP_PHYS, DUMP_LIFTED = 0, 1, 2
 OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4
 VARIANT_NARROW, VARIANT_WIDE, VARIANT_NO_BINNING, VARIANT_FORCE_BINNING, VARIANT_LATENCY = 1, 2, 4, 8, 16
 VARIANT_LAT_R2, VARIANT_LAT_R4, VARIANT_NO_TENSOR, VARIANT_AFFINE, VARIANT_NO_PREDICT = 32, 64, 128, 256, 512
-VARIANT_TENSOR32 = 1024
+VARIANT_TENSOR32, VARIANT_SMEM_MODEL = 1024, 2048
 
 EXPORTS = ("mpmi_create", "mpmi_destroy", "mpmi_step", "mpmi_step_result", "mpmi_step_sync",
-           "mpmi_step_device", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
+           "mpmi_step_device", "mpmi_step_trace", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
            "mpmi_get_info", "mpmi_strerror", "mpmi_last_error")
 
 
@@ -99,6 +99,7 @@ def load_library():
     lib.mpmi_step_result.argtypes = [vp, C.POINTER(Result)]
     lib.mpmi_step_sync.argtypes = [vp, vp, vp, u64, vp, C.POINTER(Result)]
     lib.mpmi_step_device.argtypes = [vp, vp, vp, u64, vp, vp]
+    lib.mpmi_step_trace.argtypes = [vp, vp, vp, u64, vp, vp, vp]
     lib.mpmi_shard_step.argtypes = [vp, vp, vp, u64, vp, vp]
     lib.mpmi_shard_finalize.argtypes = [vp, vp, i32, vp, u64, vp, vp]
     lib.mpmi_rollout_batch.argtypes = [vp, vp, vp, i64, i64, i32, i32, vp, vp, vp, u64, vp]
@@ -206,6 +207,9 @@ class Context:
     def step_device(self, d_x0, d_u_user, tick, stream, d_out):
         """device pointers (ints, e.g. tensor.data_ptr())"""
         self._check(self._lib.mpmi_step_device(self._h, d_x0, d_u_user, int(tick), stream, d_out))
+
+    def step_trace(self, d_x0, d_u_user, tick, stream, d_out, d_steps):
+        self._check(self._lib.mpmi_step_trace(self._h, d_x0, d_u_user, int(tick), stream, d_out, d_steps))
 
     def shard_step(self, d_x0, d_u_user, tick, stream, d_partial):
         self._check(self._lib.mpmi_shard_step(self._h, d_x0, d_u_user, int(tick), stream, d_partial))

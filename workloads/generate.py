@@ -20,6 +20,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CALIBRATION_JSON = os.path.join(_HERE, "calibration.json")
 C2_SEQUENCE = os.path.join(_HERE, "c2_tick_sequence.txt")   # written by oracle/make_c2_sequence.py
 CONFIG_NAMES = ("C1", "C2", "C3", "C4", "C5")
+# Extra parity-test workloads (not bench lines): shapes that BASELINE.json's five configs do not reach --
+# T48: lifted dim 48 (zero-padded to 64 -> the D = 64 warp-tile kernel), T4: a 4-dimensional input box (M = 4 kernels).
+TEST_NAMES = ("T48", "T4")
 
 ONE = 0xFF           # lift factor codes (include/mpmi.h: mpmi_lift_spec.terms)
 SIN, COS = 0x40, 0x80
@@ -87,7 +90,7 @@ def lift_terms(name):
     """Factor-code tables for the monomial / trig-polynomial lifts (reading G12)."""
     if name == "C1":      # x0..x3, x0^2, x0x1, x0x2, x0x3
         return _terms_from_lists([[0], [1], [2], [3], [0, 0], [0, 1], [0, 2], [0, 3]])
-    if name == "C2":      # x0..x3, the 10 products x_i x_j (i<=j), then x1^3, x3^3
+    if name in ("C2", "T4"):      # x0..x3, the 10 products x_i x_j (i<=j), then x1^3, x3^3
         return _terms_from_lists([[j] for j in range(4)] + [list(p) for p in _pairs(4)] + [[1, 1, 1], [3, 3, 3]])
     if name in ("C3", "C4"):  # (x,y,th,vx,vy,om), sin th, cos th, 21 products, vx cos, vx sin, vy cos
         return _terms_from_lists([[j] for j in range(6)] + [[SIN + 2], [COS + 2]] + [list(p) for p in _pairs(6)]
@@ -102,6 +105,8 @@ _SPEC = {
     "C3": (6, 2, 32, 10000, 60, 0.995, 1),
     "C4": (6, 2, 32, 1 << 20, 100, 0.995, 0),
     "C5": (8, 3, 128, 262144, 100, 0.99, 0),
+    "T48": (8, 3, 48, 4096, 60, 0.99, 0),
+    "T4": (4, 4, 16, 4096, 50, 0.98, 0),
 }
 _EPS_NEAR_IDENTITY = 1e-4   # C3/C4: K = S (rho (I+eps G)/rho(I+eps G)) S^-1
 
@@ -128,7 +133,7 @@ def make(name, N=None, H=None, calibrated=True, model_seed=None, gamma=None, S=N
     G = rng.standard_normal((d, d))
     Bm = 0.1 * rng.standard_normal((d, m))
     w = dict(lift_kind=0, terms=None, W=None, b=None, scale=1.0)
-    if name == "C5":
+    if name in ("C5", "T48"):
         W = rng.standard_normal((d - n, n))
         b = rng.uniform(0.0, 2.0 * np.pi, d - n)
         w.update(lift_kind=1, W=W.astype(np.float32), b=b.astype(np.float32),
@@ -148,7 +153,7 @@ def make(name, N=None, H=None, calibrated=True, model_seed=None, gamma=None, S=N
               K=K.astype(np.float32), B=Bm.astype(np.float32),
               u_lo=-np.ones(m, np.float32), u_hi=np.ones(m, np.float32),
               sampler=sampler, seed=0, rho=rho, gamma=gamma, model_seed=model_seed, **w)
-    if name in ("C1", "C2"):          # safe iff |x1| < 0.5 and |x0| < 2
+    if name in ("C1", "C2", "T4"):    # safe iff |x1| < 0.5 and |x0| < 2
         kw.update(bidx=np.array([0, 1], np.int32), blo=np.array([-2.0, -0.5], np.float32),
                   bhi=np.array([2.0, 0.5], np.float32), x_nom=np.zeros(4, np.float32),
                   x_pert=np.array([0.5, 0.1, 0.2, 0.2], np.float32))
