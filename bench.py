@@ -87,6 +87,12 @@ class ClockSampler(threading.Thread):
                 "samples": len(sm)}
 
 
+def _variant(args, mp):
+    V = mp.mpmi
+    return ((V.VARIANT_NO_TENSOR if args.no_tensor else 0) | (V.VARIANT_AFFINE if args.affine else 0) | (V.VARIANT_NO_PREDICT if args.no_predict else 0)
+            | (V.VARIANT_TENSOR32 if args.tensor32 else 0) | (V.VARIANT_TC_UNVERIFIED if args.unverified else 0))
+
+
 def _percentiles(v):
     v = np.sort(np.asarray(v, dtype=np.float64))
     return float(v[len(v) // 2]), float(v[min(len(v) - 1, int(0.99 * len(v)))])
@@ -181,7 +187,7 @@ def run_sweep(args, w_full, local):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     K_, W_ = args.steps, args.warmup
     rows = []
-    variant = (mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0) | (mp.mpmi.VARIANT_NO_PREDICT if args.no_predict else 0) | (mp.mpmi.VARIANT_TENSOR32 if args.tensor32 else 0)
+    variant = _variant(args, mp)
     for lg in range(14, 21):
         w = W.make(args.workload, N=1 << lg)
         w.noise_sigma = args.noise; w.model_kind = 1 if args.relift else 0
@@ -240,7 +246,8 @@ def main():
                     help="BASELINE.json configs[3]: N = 2^14 .. 2^20 on the chosen workload, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
                     help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
-    ap.add_argument("--tensor32", action="store_true", help="d = 32, N >= 2^17: opt-in verified tensor-core tick (3xTF32 tcgen05 rollout + FP32 second pass over the candidates near the boundary; DESIGN.md section 6)")
+    ap.add_argument("--tensor32", action="store_true", help="d = 32: take the verified tensor-core tick below 2^17 candidates too (it is the default from 2^17)")
+    ap.add_argument("--unverified", action="store_true", help="tensor-core kernels without the verification pass (measurement only: the bare 3xTF32 rollout)")
     ap.add_argument("--no-predict", action="store_true", help="d > 32: pre-sort by input-box cell instead of by predicted life time")
     ap.add_argument("--no-tensor", action="store_true", help="d = 128: FP32 SIMT tile kernel instead of the 3xTF32 tcgen05 kernel")
     ap.add_argument("--bounds-scale", type=float, default=1.0,
@@ -286,7 +293,7 @@ def main():
     from paper_1906_02318_b200.shard import shard_plan, gather_partials
     begin, count = shard_plan(w.N, 1, world, rank)             # the injected u_user (index N) goes to the last rank
     ctx = mp.Context(w, device=local, shard=(begin, count) if sharded else (0, 0),
-                     variant=(mp.mpmi.VARIANT_NO_TENSOR if args.no_tensor else 0) | (mp.mpmi.VARIANT_AFFINE if args.affine else 0) | (mp.mpmi.VARIANT_NO_PREDICT if args.no_predict else 0) | (mp.mpmi.VARIANT_TENSOR32 if args.tensor32 else 0))
+                     variant=_variant(args, mp))
     info = ctx.info()
     stream = torch.cuda.current_stream().cuda_stream
     if args.dump:

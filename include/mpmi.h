@@ -72,16 +72,16 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
        MPMI_VARIANT_SMEM_MODEL = 2048,  /* d <= 32: model staged in shared memory (LDS.128) even where the constant
                                            bank would be chosen -- the variant a context falls back to when all
                                            constant-memory slots of its device are taken                      */
-       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32, >= 2^17 candidates: VERIFIED tensor-core tick.  The
-                                           3xTF32 tcgen05 kernel (N = 32 MMAs, four CTAs per SM) rolls all
-                                           candidates; every candidate whose state came within tau of the
-                                           safe-set boundary (tau ~ 1.25e-4 x the bounds, 5-6 x the worst
-                                           3xTF32-vs-FP32 state difference) is rolled again by the FP32
-                                           register kernel, which merges its keys and finalises: flags and
-                                           winner are those of the FP32 tick.  mpmi_rollout_batch of such a
-                                           context runs the FP32 kernels.  The
-                                           environment variable MPMI_TC32_TAU_SCALE (0 < v <= 16, read by
-                                           mpmi_create) scales tau: a measurement aid, not a tuning knob     */
+       MPMI_VARIANT_TC_UNVERIFIED = 4096, /* tensor-core kernels WITHOUT the verification below: the bare 3xTF32
+                                           rollout (benchmark / test knob -- its flags are only as good as T1) */
+       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32: take the tensor-core tick below 2^17 candidates too   */
+/* The tensor-core tick (default at padded d = 128, and at padded d = 32 from 2^17 candidates; linear model) is VERIFIED:
+ * the 3xTF32 tcgen05 kernel rolls all candidates; every candidate whose state came within tau_i(k) of a safe-set
+ * boundary is rolled again by the FP32 kernel (register kernel at d = 32, warp-tile kernel at d = 128), which merges
+ * its keys and finalises, so that flags and winner are those of the FP32 tick.  tau_i(k) is a per-tick, per-step,
+ * per-dimension bound on the difference between the two arithmetics, derived from the model (csrc/bound.cuh,
+ * DESIGN.md section 6a).  The environment variable MPMI_TC_TAU_SCALE (0 <= v <= 16, read by mpmi_create) scales
+ * tau: it measures how conservative the bound is and is not a tuning knob. */
 
 /* Lift z = Psi(x).  The first n features MUST be the state itself.
  * MONO: feature f = product of up to 4 factors, codes terms[4f..4f+3]:
@@ -164,12 +164,12 @@ typedef struct {
     int32_t  d_pad;           /* internal padded lifted dim (zero rows / columns: exact)            */
     int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = warp-tile FFMA2 (d<=128),
                                  3 = latency kernel, 4 lanes per candidate (d<=32, small N),
-                                 4 = 3xTF32 tcgen05 tensor-core kernel (d_pad = 128; d_pad = 32 with MPMI_VARIANT_TENSOR32),
+                                 4 = verified 3xTF32 tcgen05 tensor-core tick (d_pad = 128; d_pad = 32 from 2^17 candidates),
                                  5 = re-lift kernel (MPMI_MODEL_RELIFT), 6 = affine-in-u kernel       */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;
     int32_t  binning_cells;   /* 0 = candidates walked in index order; else cells of the spatial pre-sort */
-    int32_t  reserved;        /* verified tensor-core tick: candidates the last finished tick handed to the FP32 pass; else 0 */
+    int32_t  reserved;        /* verified tensor-core tick: candidates the last finished mpmi_step tick handed to the FP32 pass; else 0 */
     int64_t  ncand_local;     /* candidates this context rolls out per tick                         */
 } mpmi_info;
 

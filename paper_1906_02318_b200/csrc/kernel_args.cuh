@@ -24,13 +24,14 @@ struct KArgs {
     const int *perm;                      // device, spatial order of the local sampled candidates, or null
     long long nsamp;                      // sampled candidates of this shard (perm entries)
     unsigned *work;                       // device batch counter of the persistent tile kernel (zero between launches)
-    // verified tensor-core tick (D = 32): candidates that came within tau of the safe-set boundary in the 3xTF32 rollout are
-    // not keyed there but appended to `recheck`; the FP32 register kernel (recheck_mode = 1) rolls exactly those again,
-    // merges its keys into the same TickState and finalises the tick
+    // verified tensor-core tick: candidates that came within tau_i(k) (bound.cuh) of the safe-set boundary in the 3xTF32
+    // rollout are not keyed there but appended to `recheck`; the FP32 kernel (register kernel at D = 32, warp-tile kernel at
+    // D = 128; recheck_mode = 1) rolls exactly those again, merges its keys into the same TickState and finalises the tick
     int *recheck;                         // device, kRecheckBuckets lists of capacity = local candidates each, or null
     unsigned *recheck_count;              // device, one per list; zeroed by the CTA that finalises
     int recheck_mode;                     // register kernel: 1 = walk the recheck lists (longest-lived first) instead of the index space
-    float recheck_tau_scale;              // scales tau (1 = the built-in threshold; the safety-factor measurement sets it < 1)
+    float recheck_tau_scale;              // scales tau (1 = the derived bound; MPMI_TC_TAU_SCALE < 1 measures how conservative it is)
+    int *deferred_out;                    // host-mapped: candidates the second pass rolled (mpmi_info.reserved), or null
     // batch
     const float *U;                       // device Ncand*m or null
     long long x0_count;

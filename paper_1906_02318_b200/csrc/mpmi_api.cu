@@ -22,9 +22,12 @@
 #include "mpmi_device.cuh"
 #include "kernel_args.cuh"
 #include "binning.cuh"
+#include "bound.cuh"
 
 using namespace mpmi;
 
+
+struct HostBlock { mpmi_result r; int deferred; int pad[3]; };      // mapped pinned memory the finalising CTA writes
 
 struct mpmi_ctx {
     DevCfg dc;
@@ -69,14 +72,23 @@ struct mpmi_ctx {
     int *d_pred = nullptr;
     const void *k_pred = nullptr;    // bin_predict_kernel<aff_np>
     int tc_ctas = 1;                 // persistent CTAs per SM (4 for the tensor-core kernel at D = 32)
-    // verified tensor-core tick at D = 32: the tcgen05 kernel defers the candidates that came near the safe-set boundary
-    // to the FP32 register kernel, which merges them and finalises (kernel_args.cuh: recheck)
-    KernFn k_recheck = nullptr;
+    // verified tensor-core tick: the tcgen05 kernel defers the candidates that came within tau_i(k) (bound.cuh) of the
+    // safe-set boundary to the FP32 kernel (register kernel at D = 32, warp-tile kernel at D = 128), which merges them and
+    // finalises (kernel_args.cuh: recheck).  tau comes per tick from bound_err_kernel -> bound_tau_kernel.
+    KernFn k_recheck = nullptr, k_batch_recheck = nullptr, k_batch_fp32 = nullptr;
     int *d_recheck = nullptr;
     unsigned *d_recheck_count = nullptr;
     unsigned recheck_grid = 0;
-    float recheck_tau_scale = 1.f;   // MPMI_TC32_TAU_SCALE (measurement of the threshold's safety factor only)
-    cudaGraphNode_t n_recheck = nullptr;
+    int recheck_block = kRegBlock, recheck_smem = 0;
+    bool recheck_persistent = false;
+    float recheck_tau_scale = 1.f;   // MPMI_TC_TAU_SCALE (measures how conservative the bound is; not a tuning knob)
+    cudaGraphNode_t n_recheck = nullptr, n_berr = nullptr, n_btau = nullptr;
+    const void *k_berr = nullptr, *k_btau = nullptr;
+    unsigned berr_block = 64;
+    float *d_bnd_kpow = nullptr, *d_bnd_mid = nullptr, *d_bnd_econst = nullptr, *d_bnd_w = nullptr, *d_bnd_e = nullptr, *d_bnd_tau = nullptr;
+    cudaStream_t side = nullptr;     // plain-launch entries: the bound kernels run beside the binning kernels
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int *d_deferred_mapped = nullptr;
     KArgs gr{};
     std::string err;
 };
@@ -137,6 +149,7 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
                           KernFn mpmi_pick_tilen_##D##_tick(int M, int *smem); KernFn mpmi_pick_tilen_##D##_batch(int M, int *smem);
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
+KernFn mpmi_pick_reg_32_recheck(int M); KernFn mpmi_pick_regn_32_recheck(int M);
 KernFn mpmi_pick_relift(int n, int mode);
 KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
 KernFn mpmi_pick_tc_tick(int D, int *smem, int *threads, int *ctas_per_sm, int noise); KernFn mpmi_pick_tc_batch(int D, int *smem, int *threads, int *ctas_per_sm, int noise);
@@ -241,7 +254,37 @@ const void *pick_predict(int np, int m) { return np == 4 ? pick_predict_m<4>(m) 
 unsigned pred_smem(const mpmi_ctx *c) { return (unsigned)(c->dc.H * (1 + c->dc.m) * c->dc.aff_np * 4); }
 
 #define CL(call) do { const cudaError_t e_ = (call); if (e_ != cudaSuccess) return e_; } while (0)
+// bound kernels of the verified tensor-core tick (bound.cuh): E[j][r] for this x_t, then tau_i(k)
+template <int D> const void *pick_btau(int np) {
+    return np == 4 ? (const void *)bound_tau_kernel<D, 4> : np == 8 ? (const void *)bound_tau_kernel<D, 8> : (const void *)bound_tau_kernel<D, 16>;
+}
+cudaError_t launch_bound(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {
+    void *eargs[2] = {(void *)&c->dc, (void *)&a};
+    CL(cudaLaunchKernel(c->k_berr, dim3((unsigned)c->dc.H), dim3(c->berr_block), eargs, 0, s));
+    void *targs[1] = {(void *)&c->dc};
+    return cudaLaunchKernel(c->k_btau, dim3((unsigned)c->dc.H), dim3(kBoundTauThreads), targs, 0, s);
+}
+// second pass of the verified tick / batch: the FP32 kernel over the deferral lists
+cudaError_t launch_recheck(const mpmi_ctx *c, KernFn fn, KArgs a, cudaStream_t s) {
+    a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1; a.kslot = c->kslot; a.st = c->d_state;
+    a.work = c->recheck_persistent ? &c->d_state->work : nullptr;
+    void *args[2] = {(void *)&c->dc, (void *)&a};
+    return cudaLaunchKernel((const void *)fn, dim3(c->recheck_grid), dim3((unsigned)c->recheck_block), args, (size_t)c->recheck_smem, s);
+}
+
 cudaError_t enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
+    // fork: the bound kernels need only x_t; they run on the context's side stream beside the binning kernels
+    const bool fork = c->k_recheck && c->binning;
+    if (c->k_recheck) {
+        if (fork) {
+            CL(cudaEventRecord(c->ev_fork, s));
+            CL(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+            CL(launch_bound(c, a, c->side));
+            CL(cudaEventRecord(c->ev_join, c->side));
+        } else {
+            CL(launch_bound(c, a, s));
+        }
+    }
     if (c->binning) {
         BinArgs b = c->bin;
         b.tick_val = a.tick_val;
@@ -259,13 +302,12 @@ cudaError_t enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
     if (c->affine) CL(launch_base(c, a, s));
-    if (c->k_recheck) { a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale; }
-    CL(launch(c, c->k_tick, c->dc.shard_count, a, s));
-    if (c->k_recheck) {                          // second pass: FP32 register kernel over the deferred candidates
-        a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1; a.kslot = c->kslot; a.work = nullptr;
-        void *args[2] = {(void *)&c->dc, (void *)&a};
-        CL(cudaLaunchKernel((const void *)c->k_recheck, dim3(c->recheck_grid), dim3(kRegBlock), args, 0, s));
+    if (c->k_recheck) {
+        a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale;
+        if (fork) CL(cudaStreamWaitEvent(s, c->ev_join, 0));
     }
+    CL(launch(c, c->k_tick, c->dc.shard_count, a, s));
+    if (c->k_recheck) CL(launch_recheck(c, c->k_recheck, a, s));
     return cudaSuccess;
 }
 #undef CL
@@ -303,16 +345,31 @@ void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **
 
 void recheck_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     c->gr = c->ga;                               // same inputs, sequence number and result slot as the tick node
-    c->gr.perm = nullptr; c->gr.nsamp = 0; c->gr.work = nullptr; c->gr.recheck_mode = 1;
+    c->gr.perm = nullptr; c->gr.nsamp = 0; c->gr.recheck_mode = 1;
+    c->gr.work = c->recheck_persistent ? &c->d_state->work : nullptr;
     std::memset(p, 0, sizeof *p);
     args[0] = (void *)&c->dc; args[1] = (void *)&c->gr;
-    p->func = (void *)c->k_recheck; p->gridDim = dim3(c->recheck_grid); p->blockDim = dim3(kRegBlock); p->kernelParams = args;
+    p->func = (void *)c->k_recheck; p->gridDim = dim3(c->recheck_grid); p->blockDim = dim3((unsigned)c->recheck_block);
+    p->sharedMemBytes = (unsigned)c->recheck_smem; p->kernelParams = args;
+}
+void berr_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc; args[1] = (void *)&c->ga;
+    p->func = (void *)c->k_berr; p->gridDim = dim3((unsigned)c->dc.H); p->blockDim = dim3(c->berr_block); p->kernelParams = args;
+}
+void btau_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
+    std::memset(p, 0, sizeof *p);
+    args[0] = (void *)&c->dc;
+    p->func = (void *)c->k_btau; p->gridDim = dim3((unsigned)c->dc.H); p->blockDim = dim3(kBoundTauThreads); p->kernelParams = args;
 }
 
 int build_graph(mpmi_ctx *c) {
     c->ga = KArgs{};
     c->ga.st = c->d_state; c->ga.out = c->d_res_mapped; c->ga.inline_inputs = 1; c->ga.kslot = c->kslot;
-    if (c->k_recheck) { c->ga.recheck = c->d_recheck; c->ga.recheck_count = c->d_recheck_count; c->ga.recheck_tau_scale = c->recheck_tau_scale; }
+    if (c->k_recheck) {
+        c->ga.recheck = c->d_recheck; c->ga.recheck_count = c->d_recheck_count; c->ga.recheck_tau_scale = c->recheck_tau_scale;
+        c->ga.deferred_out = c->d_deferred_mapped;
+    }
     if (c->variant == 2 || c->variant == 4) c->ga.work = &c->d_state->work;
     c->tick_grid = grid_for(c, c->dc.shard_count);
     CU(c, cudaGraphCreate(&c->graph, 0));
@@ -337,8 +394,15 @@ int build_graph(mpmi_ctx *c) {
         CU(c, cudaGraphAddKernelNode(&c->n_scatter, c->graph, &c->n_hist, 1, &p));
         dep = c->n_scatter;
     }
-    cudaGraphNode_t deps[2]; int ndep = 0;
+    cudaGraphNode_t deps[3]; int ndep = 0;
     if (dep) deps[ndep++] = dep;
+    if (c->k_recheck) {                          // bound kernels: a branch of their own beside the binning nodes
+        berr_node_params(c, &p, args);
+        CU(c, cudaGraphAddKernelNode(&c->n_berr, c->graph, nullptr, 0, &p));
+        btau_node_params(c, &p, args);
+        CU(c, cudaGraphAddKernelNode(&c->n_btau, c->graph, &c->n_berr, 1, &p));
+        deps[ndep++] = c->n_btau;
+    }
     if (c->affine) {                             // independent of the binning nodes: runs beside them
         base_node_params(c, &p, args);
         CU(c, cudaGraphAddKernelNode(&c->n_base, c->graph, nullptr, 0, &p));
@@ -383,6 +447,10 @@ void mpmi_destroy(mpmi_ctx *c) {
     cudaFree(c->d_affA); cudaFree(c->d_affG);
     cudaFree(c->d_pred);
     cudaFree(c->d_recheck); cudaFree(c->d_recheck_count);
+    cudaFree(c->d_bnd_kpow); cudaFree(c->d_bnd_mid); cudaFree(c->d_bnd_econst); cudaFree(c->d_bnd_w); cudaFree(c->d_bnd_e); cudaFree(c->d_bnd_tau);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->side) cudaStreamDestroy(c->side);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_res);
     delete c;
@@ -531,9 +599,10 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     CUC(cudaMalloc(&c->d_state, sizeof(TickState)));
     TickState st0{kKeyNone, 0ull, 0u, 0u, 0u, 0u};
     CUC(cudaMemcpy(c->d_state, &st0, sizeof st0, cudaMemcpyHostToDevice));
-    CUC(cudaHostAlloc(&c->h_res, sizeof(mpmi_result), cudaHostAllocMapped));
-    std::memset(c->h_res, 0, sizeof(mpmi_result));
+    CUC(cudaHostAlloc(&c->h_res, sizeof(HostBlock), cudaHostAllocMapped));       // the result, then the second pass's count
+    std::memset(c->h_res, 0, sizeof(HostBlock));
     CUC(cudaHostGetDevicePointer((void **)&c->d_res_mapped, c->h_res, 0));
+    c->d_deferred_mapped = &reinterpret_cast<HostBlock *>(c->d_res_mapped)->deferred;
 
     // ---- spatial binning: large Philox candidate sets only (the grid is already spatially ordered)
     {
@@ -564,6 +633,14 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     // the latency kernel does not carry it, so sigma != 0 routes around it
     const bool noise = cfg->noise_sigma != 0.f;
     dc.noise_sigma = cfg->noise_sigma; dc.model = cfg->model;
+    const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16;
+    const size_t aff_smem = (size_t)cfg->H * (1 + m) * NPn * sizeof(float);
+    // tensor cores: linear lifted model only; noise block holds 8 dims; the verification tables (bound.cuh) must fit
+    const bool tc_unverified = (cfg->variant & MPMI_VARIANT_TC_UNVERIFIED) != 0;
+    const bool tc_model_ok = cfg->model == MPMI_MODEL_LINEAR && (!noise || n <= 8) &&
+                             !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_AFFINE)) &&
+                             (tc_unverified || ((size_t)cfg->H * D * D * sizeof(float) <= ((size_t)256 << 20) && aff_smem <= 200 * 1024));
+    bool tensor = false, tc32_batch = false;
     if (cfg->model == MPMI_MODEL_RELIFT) {
         // x' = C (K Psi(x) + B u): one thread per candidate, only the physical rows of the model (rollout_relift.cuh)
         c->variant = 5;
@@ -596,7 +673,9 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         c->k_batch = pick_reg(D, M, c->P, MODE_BATCH, noise, kconst_batch);
         c->k_batch_dump = pick_reg(D, M, 1, MODE_BATCH, noise, kconst_batch);
         // paper-scale candidate sets: 4 lanes per candidate (rollout_lat.cuh) shorten the dependent chain
-        const bool lat = !noise && ((cfg->variant & MPMI_VARIANT_LATENCY) || (!(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE)) && sc <= kLatMaxCand));
+        const bool force_tc32 = D == 32 && tc_model_ok && (cfg->variant & MPMI_VARIANT_TENSOR32) &&
+                                !(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY | MPMI_VARIANT_SMEM_MODEL));
+        const bool lat = !noise && !force_tc32 && ((cfg->variant & MPMI_VARIANT_LATENCY) || (!(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE)) && sc <= kLatMaxCand));
         if (lat && !c->binning) {
             // rows per lane: 2 (D/2 lanes per candidate) while that still leaves SMs short of warps, else 4
             const long long warps_r4 = sc * (D / 4) / 32;
@@ -606,35 +685,31 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             c->k_tick = pick_lat(D, M, R);
             c->block = 64; c->cand_per_block = 64 / (D / R);     // D/R lanes per candidate
         }
-        // D = 32, large candidate sets, on request (MPMI_VARIANT_TENSOR32: its flags are not within the 1e-4 margin rule at
-        // large state magnitudes): the same 3xTF32 tcgen05 kernel as at d = 128, with N = 32 MMAs and four CTAs per SM
-        if (D == 32 && c->variant == 1 && (cfg->variant & MPMI_VARIANT_TENSOR32) && sc >= kTc32MinCand && (!noise || n <= 8) &&
-            !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY | MPMI_VARIANT_AFFINE))) {
-            // The tick is VERIFIED: candidates whose 3xTF32 state came near the safe-set boundary are rolled again by the
-            // FP32 register kernel (2 candidates per thread), so flags and winner are those of the FP32 path.  The batch
-            // entry stays on the FP32 register kernels chosen above.
+        // D = 32, large candidate sets: the 3xTF32 tcgen05 kernel of d = 128 with N = 32 MMAs and four CTAs per SM, as a
+        // VERIFIED tick (below).  The batch entry stays on the FP32 register kernels chosen above.
+        if (D == 32 && c->variant == 1 && tc_model_ok && (sc >= kTc32MinCand || (cfg->variant & MPMI_VARIANT_TENSOR32)) &&
+            !(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY | MPMI_VARIANT_SMEM_MODEL))) {
+            tensor = true;
             c->variant = 4;
-            int threads = 0, bs = 0, bt = 0, bc = 0;
+            int threads = 0;
             c->k_tick = mpmi_pick_tc_tick(D, &c->smem, &threads, &c->tc_ctas, noise);
-            (void)mpmi_pick_tc_batch(D, &bs, &bt, &bc, noise);
             c->block = threads; c->cand_per_block = 128;
             CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
-            // the second pass sees a few 10^4 candidates: below ~2^19 the shared-memory model is the faster one (section 9 sweep)
-            c->k_recheck = pick_reg(D, M, 1, MODE_TICK, noise, 0);
-            c->recheck_grid = (unsigned)((sc + 2 * kRegBlock - 1) / (2 * kRegBlock));
-            CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc * kRecheckBuckets));
-            CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned) * kRecheckBuckets));
-            CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned) * kRecheckBuckets));
-            if (const char *e = std::getenv("MPMI_TC32_TAU_SCALE")) {
-                const float v = (float)std::atof(e);
-                if (v > 0.f && v <= 16.f) c->recheck_tau_scale = v;
+            if (tc_unverified) {         // measurement knob: the bare tensor-core kernel serves the batch entry as well
+                int bs = 0, bt = 0, bc = 0;
+                c->k_batch = mpmi_pick_tc_batch(D, &bs, &bt, &bc, noise);
+                c->k_batch_dump = nullptr;
+                c->bblock = bt; c->bcand_per_block = 128; tc32_batch = true;
+                CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
             }
         }
     } else {
-        // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh)
+        // d = 128: the step is a dense contraction -> 3xTF32 on the tcgen05 tensor cores (rollout_tc.cuh), verified (below),
         // unless the caller asks for the FP32 SIMT tile kernel; d = 64 stays on the SIMT tile kernel
-        const bool tensor = D == 128 && (!noise || n <= 8) && !(cfg->variant & MPMI_VARIANT_NO_TENSOR);   // its noise block holds 8 dims
+        tensor = D == 128 && tc_model_ok;
         c->P = 1;
+        int fsmem = 0;
+        c->k_batch_fp32 = pick_tile(D, M, MODE_BATCH, &fsmem, noise);
         if (tensor) {
             c->variant = 4;
             int threads = 0;
@@ -645,21 +720,22 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             c->variant = 2;
             c->block = kTileThreads; c->cand_per_block = kTileNC;
             c->k_tick = pick_tile(D, M, MODE_TICK, &c->smem, noise);
-            c->k_batch = pick_tile(D, M, MODE_BATCH, &c->smem, noise);
+            c->k_batch = c->k_batch_fp32;
         }
         c->bblock = c->block; c->bcand_per_block = c->cand_per_block;
         if (c->k_tick) {
             CUC(cudaFuncSetAttribute((const void *)c->k_tick, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
             CUC(cudaFuncSetAttribute((const void *)c->k_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem));
+            CUC(cudaFuncSetAttribute((const void *)c->k_batch_fp32, cudaFuncAttributeMaxDynamicSharedMemorySize, fsmem));
         }
     }
-    c->bsmem = c->k_recheck ? 0 : c->smem;
-    c->bpersistent = (c->variant == 2 || c->variant == 4) && !c->k_recheck;
+    c->bsmem = (D <= 32 && !tc32_batch) ? 0 : c->smem;
+    c->bpersistent = (c->variant == 2 || c->variant == 4) && (D > 32 || tc32_batch);
     // x_k = a_k + G_k u: tabulate G_k = C S_k B, S_k = sum_{i<k} K^i, in FP64 (T_1 = B, T_{k+1} = K T_k + B); a_k comes per tick
     // from affine_base_kernel.  Used by the affine variant and by the life-time order of the tile kernels.
-    const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16;
-    const size_t aff_smem = (size_t)cfg->H * (1 + m) * NPn * sizeof(float);
+    bool affine_built = false;
     auto build_affine = [&]() -> int {
+        affine_built = true;
         const int Hh = cfg->H;
         std::vector<double> T((size_t)d * m), Tn((size_t)d * m);
         std::vector<float> G((size_t)Hh * m * NPn, 0.f);
@@ -724,6 +800,115 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         CUC(cudaFuncSetAttribute(c->k_pred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
         c->bin.keys = c->d_pred; c->bin.H = cfg->H; c->bin.ncells = cfg->H + 1;
     }
+    // ---- verified tensor-core tick: second-pass kernel, deferral lists, bound tables (bound.cuh) -----------------------------
+    if (tensor && c->variant == 4 && !tc_unverified) {
+        if (!affine_built) { rc = build_affine(); if (rc != MPMI_OK) return bail(rc); }
+        if (D == 32) {               // FP32 register kernel, 2 candidates per thread, CTAs loop over blocks of the lists
+            c->k_recheck = noise ? mpmi_pick_regn_32_recheck(M) : mpmi_pick_reg_32_recheck(M);
+            c->recheck_block = kRegBlock; c->recheck_smem = 0; c->recheck_persistent = false;
+            const long long nb = (sc + 2 * kRegBlock - 1) / (2 * kRegBlock), cap = 3LL * c->sm_count;
+            c->recheck_grid = (unsigned)(nb < cap ? nb : cap);
+        } else {                     // FP32 warp-tile kernel, persistent CTAs fetch batches of the lists from the work counter
+            c->k_recheck = pick_tile(D, M, MODE_TICK, &c->recheck_smem, noise);
+            c->k_batch_recheck = c->k_batch_fp32;
+            c->recheck_block = kTileThreads; c->recheck_persistent = true;
+            const long long nb = (sc + kTileNC - 1) / kTileNC;
+            c->recheck_grid = (unsigned)(nb < c->sm_count ? nb : c->sm_count);
+            CUC(cudaFuncSetAttribute((const void *)c->k_recheck, cudaFuncAttributeMaxDynamicSharedMemorySize, c->recheck_smem));
+        }
+        if (!c->k_recheck) { c->err = "no second-pass kernel for this (d, m)"; return bail(MPMI_ERR_UNSUPPORTED); }
+        CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc * kRecheckBuckets));
+        CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned) * kRecheckBuckets));
+        CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned) * kRecheckBuckets));
+        if (const char *e = std::getenv("MPMI_TC_TAU_SCALE")) {
+            const float v = (float)std::atof(e);
+            if (v >= 0.f && v <= 16.f) c->recheck_tau_scale = v;
+        }
+        CUC(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+        CUC(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        CUC(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+
+        // -- tables, FP64, internal order (Kin[r][c] = KTa[c][r], Bin[r][j] = KTa[D + j][r])
+        const int Hh = cfg->H;
+        const double u24 = std::ldexp(1.0, -24);
+        const int KB = D / 8;
+        // column weights w_c of the per-step error bound E_r = sum_c w_c |K_rc| |z_c| (bound.cuh):
+        //   FP32 kernel: term c passes through (D + M - c) roundings of 2^-24 each (+1 when sigma*eps is added afterwards);
+        //   3xTF32 operands: z_lo K_lo dropped (|z_lo| < 2^-10 |z|, |K_lo| < 2^-10 |K|: 2^-20) + z_lo and K_lo rounded to TF32
+        //   (relative 2^-11 of a 2^-10 part: 2^-21 each) = 2^-19;
+        //   tensor-core accumulation: <= 2 ulp = 2^-22 of the running sum per MMA, for the Z_hi K_hi MMAs from column c's
+        //   k-block on (input block last, then the noise block); the 2 KB + 3 small-product MMAs before them run on sums
+        //   below 2^-9 of the full magnitude: 2^-31 each.
+        std::vector<float> wv((size_t)D + M, 0.f);
+        const int nblk = KB + 1 + (noise ? 1 : 0), nfp = D + M + (noise ? 1 : 0);
+        for (int cc = 0; cc < D + M; cc++) {
+            const int blk = cc < D ? cc / 8 : KB;
+            wv[cc] = (float)(u24 * (nfp - cc) + std::ldexp(1.0, -19) + std::ldexp(1.0, -22) * (nblk - blk) + std::ldexp(1.0, -31) * (2 * KB + 3));
+        }
+        const double wnoise = u24 + std::ldexp(1.0, -20) + std::ldexp(1.0, -22);      // the sigma*eps column: one FP32 rounding, hi/lo split, one MMA
+        const double epsmax = 5.77;                                                    // Box-Muller with u1 >= 2^-24: |eps| <= sqrt(48 ln 2) = 5.768
+        std::vector<double> Kin((size_t)D * D), Bin((size_t)D * M);
+        for (int r = 0; r < D; r++) {
+            for (int cc = 0; cc < D; cc++) Kin[(size_t)r * D + cc] = KTa[(size_t)cc * D + r];
+            for (int j = 0; j < M; j++) Bin[(size_t)r * M + j] = KTa[(size_t)(D + j) * D + r];
+        }
+        std::vector<double> umid(M), uhalf(M), umax(M);
+        for (int j = 0; j < M; j++) {
+            umid[j] = 0.5 * ((double)cfg->u_lo[j] + cfg->u_hi[j]); uhalf[j] = 0.5 * ((double)cfg->u_hi[j] - cfg->u_lo[j]);
+            umax[j] = std::fmax(std::fabs((double)cfg->u_lo[j]), std::fabs((double)cfg->u_hi[j]));
+        }
+        std::vector<double> Kp((size_t)D * D, 0.0), Kn((size_t)D * D), T((size_t)D * M, 0.0), Tn((size_t)D * M), nz(D, 0.0), zabs(D);
+        for (int r = 0; r < D; r++) Kp[(size_t)r * D + r] = 1.0;
+        std::vector<float> kpowT((size_t)Hh * D * D), mid((size_t)Hh * D), econst((size_t)Hh * D);
+        for (int j = 0; j < Hh; j++) {
+            float *kt = &kpowT[(size_t)j * D * D];
+            for (int r = 0; r < D; r++) for (int cc = 0; cc < D; cc++) kt[(size_t)cc * D + r] = (float)Kp[(size_t)r * D + cc];
+            for (int r = 0; r < D; r++) {                       // z_j over the input box: centre (S_j B) u_mid, half-width |S_j B| u_half
+                double mv = 0.0, av = 0.0;
+                for (int i = 0; i < M; i++) { mv += T[(size_t)r * M + i] * umid[i]; av += std::fabs(T[(size_t)r * M + i]) * uhalf[i]; }
+                mid[(size_t)j * D + r] = (float)mv;
+                zabs[r] = av + (noise ? epsmax * (double)cfg->noise_sigma * nz[r] : 0.0);
+            }
+            for (int r = 0; r < D; r++) {
+                double e = 0.0;
+                for (int cc = 0; cc < D; cc++) e += (double)wv[cc] * std::fabs(Kin[(size_t)r * D + cc]) * zabs[cc];
+                for (int i = 0; i < M; i++) e += (double)wv[D + i] * std::fabs(Bin[(size_t)r * M + i]) * umax[i];
+                if (noise && r < n) e += wnoise * epsmax * (double)cfg->noise_sigma;
+                econst[(size_t)j * D + r] = (float)(e * (1.0 + 1e-6));
+            }
+            if (j + 1 == Hh) break;
+            if (noise) for (int r = 0; r < D; r++) for (int i = 0; i < n; i++) nz[r] += std::fabs(Kp[(size_t)r * D + i]);   // sum_{p<=j} |K^p E|
+            std::fill(Kn.begin(), Kn.end(), 0.0);              // K^{j+1} = K K^j,  S_{j+1} B = K (S_j B) + B
+            for (int r = 0; r < D; r++)
+                for (int q = 0; q < D; q++) {
+                    const double v = Kin[(size_t)r * D + q];
+                    if (v != 0.0) for (int cc = 0; cc < D; cc++) Kn[(size_t)r * D + cc] += v * Kp[(size_t)q * D + cc];
+                }
+            Kp.swap(Kn);
+            for (int r = 0; r < D; r++)
+                for (int i = 0; i < M; i++) {
+                    double v = Bin[(size_t)r * M + i];
+                    for (int q = 0; q < D; q++) v += Kin[(size_t)r * D + q] * T[(size_t)q * M + i];
+                    Tn[(size_t)r * M + i] = v;
+                }
+            T.swap(Tn);
+        }
+        auto up = [&](float **dst, const std::vector<float> &src) -> int {
+            CU(c, cudaMalloc(dst, src.size() * sizeof(float)));
+            CU(c, cudaMemcpy(*dst, src.data(), src.size() * sizeof(float), cudaMemcpyHostToDevice));
+            return MPMI_OK;
+        };
+        if ((rc = up(&c->d_bnd_kpow, kpowT)) != MPMI_OK || (rc = up(&c->d_bnd_mid, mid)) != MPMI_OK ||
+            (rc = up(&c->d_bnd_econst, econst)) != MPMI_OK || (rc = up(&c->d_bnd_w, wv)) != MPMI_OK) return bail(rc);
+        CUC(cudaMalloc(&c->d_bnd_e, (size_t)Hh * D * sizeof(float)));
+        CUC(cudaMalloc(&c->d_bnd_tau, (size_t)(Hh + 1) * (NPn + kTauPad) * sizeof(float)));
+        CUC(cudaMemset(c->d_bnd_tau, 0, (size_t)(Hh + 1) * (NPn + kTauPad) * sizeof(float)));
+        dc.bnd_kpow = c->d_bnd_kpow; dc.bnd_mid = c->d_bnd_mid; dc.bnd_econst = c->d_bnd_econst; dc.bnd_w = c->d_bnd_w;
+        dc.bnd_e = c->d_bnd_e; dc.bnd_tau = c->d_bnd_tau;
+        c->k_berr = D == 32 ? (const void *)bound_err_kernel<32> : (const void *)bound_err_kernel<128>;
+        c->berr_block = D < 64 ? 64 : (unsigned)D;
+        c->k_btau = D == 32 ? pick_btau<32>(NPn) : pick_btau<128>(NPn);
+    }
     if (!c->k_tick || !c->k_batch) { c->err = "no kernel for this (d, m)"; return bail(MPMI_ERR_UNSUPPORTED); }
     cudaFuncAttributes fa;
     CUC(cudaFuncGetAttributes(&fa, (const void *)c->k_tick));
@@ -742,11 +927,11 @@ int mpmi_get_info(const mpmi_ctx *c, mpmi_info *o) {
     o->threads_per_block = c->block;
     o->blocks = (int)grid_for(c, c->dc.shard_count);
     o->smem_bytes = c->smem + (c->variant == 1 ? (c->dc.D + c->dc.m + 1) * c->dc.D * 4 : 0);
-    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0) + (c->predict ? 1 : 0) + (c->k_recheck ? 1 : 0); o->uses_graph = 1;
+    o->regs_per_thread = c->regs; o->sm_count = c->sm_count; o->launches_per_tick = (c->binning ? 3 : 1) + (c->affine ? 1 : 0) + (c->predict ? 1 : 0) + (c->k_recheck ? 3 : 0); o->uses_graph = 1;
     o->binning_cells = c->binning ? c->bin.ncells : 0;
     o->ncand_local = c->dc.shard_count;
-    if (c->k_recheck)                            // candidates the last finished tick handed to the FP32 pass
-        cudaMemcpy(&o->reserved, &c->d_state->pad, sizeof(int), cudaMemcpyDeviceToHost);
+    if (c->k_recheck)                            // candidates the last finished HOST-path tick handed to the FP32 pass (mapped
+        o->reserved = *reinterpret_cast<volatile const int *>(&reinterpret_cast<const HostBlock *>(c->h_res)->deferred);   // memory: no sync)
     return MPMI_OK;
 }
 
@@ -782,6 +967,8 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     if (c->k_recheck) {
         recheck_node_params(c, &p, args);
         CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_recheck, &p));
+        berr_node_params(c, &p, args);
+        CU(c, cudaGraphExecKernelNodeSetParams(c->exec, c->n_berr, &p));
     }
     CU(c, cudaGraphLaunch(c->exec, (cudaStream_t)stream));
     c->pending = true; c->pending_stream = (cudaStream_t)stream;
@@ -884,6 +1071,20 @@ int mpmi_rollout_batch(mpmi_ctx *c, const float *d_U, const float *d_X0, int64_t
         CU(c, launch(c, c->k_batch_aff, Ncand, a, (cudaStream_t)stream));
     } else if (dump_kind != MPMI_DUMP_NONE && c->k_batch_dump && c->variant != 5) {
         CU(c, launch_geom(c, c->k_batch_dump, Ncand, a, (cudaStream_t)stream, 256, 128, 0, false));
+    } else if (c->k_batch_recheck) {
+        // d = 128, verified context.  The bound tau_i(k) is taken over the context's input box, horizon and one x_t, so the
+        // tensor-core batch applies to the internal sampler with a shared x0 (first pass: 3xTF32, every candidate; second
+        // pass: the FP32 warp-tile kernel rewrites steps / flags / dumped states of the deferred ones); caller-supplied
+        // inputs, per-candidate x0 or a longer horizon run on the FP32 warp-tile kernel alone.
+        if (!d_U && x0_count == 1 && H <= c->dc.H && Ncand <= c->dc.shard_count) {
+            cudaStream_t s = (cudaStream_t)stream;
+            CU(c, launch_bound(c, a, s));
+            a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale;
+            CU(c, launch(c, c->k_batch, Ncand, a, s));
+            CU(c, launch_recheck(c, c->k_batch_recheck, a, s));
+        } else {
+            CU(c, launch_geom(c, c->k_batch_fp32, Ncand, a, (cudaStream_t)stream, kTileNC, kTileThreads, c->recheck_smem, true));
+        }
     } else {
         CU(c, launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream));
     }

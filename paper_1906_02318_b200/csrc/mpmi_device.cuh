@@ -41,6 +41,13 @@ struct DevCfg {
     const float *aff_g;             // device: H x m x aff_np, from mpmi_create (FP64 -> fp32)
     const float *aff_m;             // device: H x aff_np x D, rows of C K^k (FP64 -> fp32)
     int aff_np;                     // padded physical dim: 4, 8 or 16
+    // verified tensor-core tick (bound.cuh): tables of mpmi_create (FP64 -> fp32) and the two per-tick results
+    const float *bnd_kpow;          // device: H x D x D, kpowT[j][c][r] = (K^j)[r][c], internal order
+    const float *bnd_mid;           // device: H x D, (S_j B) u_mid
+    const float *bnd_econst;        // device: H x D, tick-independent part of the per-step error bound E
+    const float *bnd_w;             // device: D + M column weights w_c of E
+    float *bnd_e;                   // device: H x D, E[j][r] of this tick (bound_err_kernel)
+    float *bnd_tau;                 // device: (H + 1) x (aff_np + 4), tau_i(k) of this tick (bound_tau_kernel)
 };
 
 // Cross-block selection state; reset by the block that finalises the tick.
@@ -242,7 +249,8 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
                                                           unsigned n_safe, unsigned long long n_exec,
                                                           unsigned long long tick, const float (&u_h)[kMaxM],
                                                           TickState *st, mpmi_result *out, mpmi_partial *partial,
-                                                          unsigned seq = 0, unsigned *work = nullptr, bool defer = false, int nwork = 1) {
+                                                          unsigned seq = 0, unsigned *work = nullptr, bool defer = false,
+                                                          unsigned *lists = nullptr, int nlists = 0, int *deferred_out = nullptr) {
     __shared__ unsigned long long s_key[kWarps];
     __shared__ unsigned s_safe[kWarps];
     __shared__ unsigned long long s_exec[kWarps];
@@ -276,17 +284,19 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
             const unsigned long long bk = atomicMin(&st->best_key, kKeyNone);     // atomic read
             const unsigned long long tot_exec = atomicAdd(&st->n_exec, 0ull);
             const unsigned tot_safe = atomicAdd(&st->n_safe, 0u);
+            if (lists) {                 // second pass of a verified tick: empty the deferral lists, report how many it rolled
+                unsigned tot = 0;
+                for (int i = 0; i < nlists; i++) { tot += lists[i]; lists[i] = 0u; }
+                st->pad = tot;
+                if (deferred_out) *reinterpret_cast<volatile int *>(deferred_out) = (int)tot;     // (mapped: before the sequence number)
+            }
             if (partial) {
                 partial->key = bk; partial->n_safe = tot_safe; partial->n_exec = (long long)tot_exec;
             } else {
                 decode_result(cfg, bk, tot_exec, tot_safe, tick, u_h, out, seq);
             }
             st->best_key = kKeyNone; st->n_exec = 0ull; st->n_safe = 0u; st->ticket = 0u;   // ready for next tick
-            if (work) {
-                unsigned tot = 0;
-                for (int i = 0; i < nwork; i++) { tot += work[i]; work[i] = 0u; }
-                st->pad = tot;
-            }
+            if (work) *work = 0u;
             __threadfence();
         }
     }

@@ -26,9 +26,12 @@ constexpr int reg_min_blocks() { return (D * P >= 32) ? 3 : 4; }
 // KC = true: model values from the constant bank (slot a.kslot of c_model), the choice for grids that fill the machine;
 // KC = false: staged in shared memory and read with warp-uniform LDS.128 -- better when an SM holds only one or two
 // warps, which cannot hide the constant-cache misses of a 4.3 KB model (measured crossover: ~2^19 candidates at D = 32).
-template <int D, int M, int P, int MODE, bool NOISE = false, bool KC = true>
+// RC = true: second pass of the verified tensor-core tick (kernel_args.cuh): the CTAs walk the deferral lists (longest-lived
+// first) in blocks of 2P * blockDim candidates, block b of CTA x = x + b * gridDim, and the last CTA finalises the tick.
+template <int D, int M, int P, int MODE, bool NOISE = false, bool KC = true, bool RC = false>
 __global__ void __launch_bounds__(kRegBlock, reg_min_blocks<D, P>())
 rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
+    static_assert(!RC || MODE == MODE_TICK, "the second pass is a tick kernel");
     constexpr int S = 2 * P;                 // candidates per thread
     constexpr int NB = D < kMaxN ? D : kMaxN;
     __shared__ __align__(16) float sK[KC ? 4 : (D + M) * D];
@@ -59,6 +62,12 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     }
     __syncthreads();
 
+    unsigned long long key = kKeyNone;
+    unsigned n_safe = 0, n_exec = 0;
+    int rc_count[kRecheckBuckets], rc_total = 0;
+#pragma unroll
+    for (int b = 0; b < kRecheckBuckets; b++) { rc_count[b] = RC ? (int)a.recheck_count[b] : 0; rc_total += rc_count[b]; }
+  for (long long blk = blockIdx.x; !RC || blk * (2 * P * (long long)blockDim.x) < rc_total; blk += gridDim.x) {
     // ---- a1 + a2: candidates of this thread ------------------------------------------------------
     float2 z[P][D + M];
     long long li[S];
@@ -67,15 +76,15 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
     for (int s = 0; s < S; s++) {
         // the two halves of a register pair are ADJACENT candidates (2*tid, 2*tid+1): dumps store float2
-        li[s] = (long long)blockIdx.x * (S * bdim) + (s >> 1) * (2 * bdim) + 2 * tid + (s & 1);
-        if (MODE == MODE_TICK && a.perm && li[s] < a.nsamp) li[s] = a.perm[li[s]];   // spatially ordered walk
-        if (MODE == MODE_TICK && a.recheck_mode) {                                    // second pass of the verified tensor-core tick
-            long long p = li[s], hit = ncand;                                         // slot p of the concatenated lists
+        li[s] = blk * (S * bdim) + (s >> 1) * (2 * bdim) + 2 * tid + (s & 1);
+        if (MODE == MODE_TICK && !RC && a.perm && li[s] < a.nsamp) li[s] = a.perm[li[s]];   // spatially ordered walk
+        if (RC) {                                                                     // second pass of the verified tensor-core tick
+            int p = (int)li[s];                                                       // slot p of the concatenated lists
+            long long hit = ncand;
 #pragma unroll
             for (int b = 0; b < kRecheckBuckets; b++) {
-                const long long cb = (long long)a.recheck_count[b];
-                if (p >= 0 && p < cb) hit = (long long)a.recheck[(long long)b * ncand + p];
-                p -= cb;                                                              // negative once the slot has been found
+                if (p >= 0 && p < rc_count[b]) hit = (long long)a.recheck[(long long)b * ncand + p];
+                p -= rc_count[b];                                                     // negative once the slot has been found
             }
             li[s] = hit;
         }
@@ -121,7 +130,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
     const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
     const bool vec2 = dump && (ncand % 2 == 0) && ((reinterpret_cast<unsigned long long>(a.traj) & 7ull) == 0);
-    const bool dump_fast = vec2 && ((long long)(blockIdx.x + 1) * (S * bdim) <= ncand) && ((long long)J * ncand < (1ll << 31));
+    const bool dump_fast = vec2 && ((blk + 1) * (S * bdim) <= ncand) && ((long long)J * ncand < (1ll << 31));
     const bool dump_full = J == D;           // lifted dump of an unpadded model: every row is stored
     unsigned dump_row[NB];                   // original row of internal row j (only the first n are permuted)
 #pragma unroll
@@ -266,8 +275,6 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     }
 
     // ---- a5-a7: key, argmin, finalise -------------------------------------------------------------
-    unsigned long long key = kKeyNone;
-    unsigned n_safe = 0, n_exec = 0;
 #pragma unroll
     for (int s = 0; s < S; s++) {
         if (a.steps && li[s] < ncand) a.steps[li[s]] = steps[s];   // mpmi_step_trace: per-candidate steps of THIS tick kernel
@@ -286,8 +293,10 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
             n_exec += (unsigned)(steps[s] + 1 < H ? steps[s] + 1 : H);
         }
     }
-    block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq,
-                                              (MODE == MODE_TICK && a.recheck_mode) ? a.recheck_count : nullptr, false, kRecheckBuckets);
+    if (!RC) break;
+  }
+    block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, nullptr, false,
+                                              RC ? a.recheck_count : nullptr, kRecheckBuckets, a.deferred_out);
 }
 
 }  // namespace mpmi

@@ -115,27 +115,40 @@ __device__ __forceinline__ bool safe_check_par(const DevCfg &cfg, const float (&
     return ok;
 }
 
-// Verified tick (D = 32): did this state come within tau of the safe-set boundary (on either side)?  The 3xTF32 rollout is
-// within ~2e-5 relative of the FP32 one, so a candidate that never does has the same flags in both; one that does is
-// rolled again by the FP32 register kernel (kernel_args.cuh: recheck).  tau_box in state units, tau_ann2 in r^2 units.
+// Verified tick: did this state come within tau_i(k) of the safe-set boundary (on either side)?  tau_i(k) (bound.cuh) bounds
+// |x~_k - x^_k|_i between this kernel's state and the FP32 kernel's for the same candidate, so a candidate that never does has,
+// step by step, the same isSafe result in both; one that does is rolled again by the FP32 kernel (kernel_args.cuh: recheck).
+// trow = this step's row of the tau table: [tau_0 .. tau_{np-1} | thr(r_min^2), thr(r_max^2)].  NaN counts as near.
+template <int NB, int J0, int J1>
+__device__ __forceinline__ float box_near(const DevCfg &cfg, const float (&x)[NB], const float *trow, float sc) {
+    if constexpr (J1 - J0 == 1) {
+        const float q = fminf(fabsf(__fsub_rn(x[J0], cfg.blo[J0])), fabsf(__fsub_rn(cfg.bhi[J0], x[J0])));
+        return __fmaf_rn(-sc, __ldg(trow + J0), q);                    // distance to the nearer limit, minus tau
+    } else {
+        constexpr int JM = (J0 + J1) / 2;
+        return min_nan(box_near<NB, J0, JM>(cfg, x, trow, sc), box_near<NB, JM, J1>(cfg, x, trow, sc));
+    }
+}
 template <int NB>
-__device__ __forceinline__ bool near_boundary(const DevCfg &cfg, const float (&x)[NB], int nbox, float tau_box, float tau_ann2) {
+__device__ __forceinline__ bool near_boundary(const DevCfg &cfg, const float (&x)[NB], int nbox, const float *trow, int np, float sc) {
     bool nr = false;
     if (nbox > 0) {
-        float m = box_slack<NB, 0, 2>(cfg, x);
+        float m = box_near<NB, 0, 2>(cfg, x, trow, sc);
         if (nbox > 2) {
-            m = min_nan(m, box_slack<NB, 2, 4>(cfg, x));
+            m = min_nan(m, box_near<NB, 2, 4>(cfg, x, trow, sc));
             if (nbox > 4) {
-                m = min_nan(m, box_slack<NB, 4, 8>(cfg, x));
-                if (nbox > 8) m = min_nan(m, box_slack<NB, 8, 16>(cfg, x));
+                m = min_nan(m, box_near<NB, 4, 8>(cfg, x, trow, sc));
+                if (nbox > 8) m = min_nan(m, box_near<NB, 8, 16>(cfg, x, trow, sc));
             }
         }
-        nr = fabsf(m) < tau_box;
+        nr = !(m >= 0.f);
     }
     if (cfg.annulus) {
         const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
         const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
-        nr = nr || fabsf(fminf(__fsub_rn(r2, cfg.rmin2), __fsub_rn(cfg.rmax2, r2))) < tau_ann2;
+        const float qa = __fmaf_rn(-sc, __ldg(trow + np), fabsf(__fsub_rn(r2, cfg.rmin2)));
+        const float qb = __fmaf_rn(-sc, __ldg(trow + np + 1), fabsf(__fsub_rn(cfg.rmax2, r2)));
+        nr = nr || !(min_nan(qa, qb) >= 0.f);
     }
     return nr;
 }
@@ -319,21 +332,10 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         const bool dump = (MODE == MODE_BATCH) && a.dump_kind != MPMI_DUMP_NONE;
         const int J = dump ? (a.dump_kind == MPMI_DUMP_PHYS ? cfg.n : cfg.d) : 0;
         const float qnan = __int_as_float(0x7fc00000);
-        // verified tick: tau = 1.25e-4 x the size of the bounds (>= 1e-3).  Measured on C4 (|x| ~ 10, |z| ~ 130, bounds 12) with
-        // MPMI_TC32_TAU_SCALE over 40 ticks x 2^20 candidates: the result equals the FP32 tick's down to tau = 2.9e-4 and
-        // first differs at 2.5e-4 (the largest 3xTF32-vs-FP32 state difference that decides a flag), so tau = 1.5e-3 there is
-        // 5-6x that; ~6.5 % of the candidates take the second pass
-        const bool verify = (D == 32) && (MODE == MODE_TICK) && a.recheck != nullptr;
-        float tau_box = 1e-3f, tau_ann2 = 0.f;
-        if (verify) {
-            for (int j = 0; j < nbox && j < NB; j++) {
-                if (isfinite(cfg.blo[j])) tau_box = fmaxf(tau_box, 1.25e-4f * fabsf(cfg.blo[j]));
-                if (isfinite(cfg.bhi[j])) tau_box = fmaxf(tau_box, 1.25e-4f * fabsf(cfg.bhi[j]));
-            }
-            const float rmax = sqrtf(cfg.rmax2);
-            tau_box *= a.recheck_tau_scale;
-            tau_ann2 = 2.f * rmax * fmaxf(1e-3f, 1.25e-4f * rmax) * a.recheck_tau_scale;
-        }
+        // verified tick / batch: a.recheck != null -- candidates that come within tau_i(k) of the boundary go to the FP32 kernel
+        const bool verify = a.recheck != nullptr;
+        const int tau_stride = cfg.aff_np + 4;                       // bound.cuh: kTauPad
+        const float tau_sc = a.recheck_tau_scale;
         unsigned p_full = 0, p_tile = 0;
 #ifdef MPMI_TC_DEBUG
         long long sw_wait = 0, sw_ld = 0, sw_math = 0, sw_st = 0, sw_n = 0, sw_skew = 0, sq = clock64();
@@ -468,7 +470,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     float x[NB];
 #pragma unroll
                     for (int j = 0; j < NB; j++) x[j] = __uint_as_float(r[j]);
-                    near = near || (was_alive && near_boundary<NB>(cfg, x, nbox, tau_box, tau_ann2));
+                    near = near || (was_alive && near_boundary<NB>(cfg, x, nbox, cfg.bnd_tau + (size_t)s * tau_stride, cfg.aff_np, tau_sc));
                 }
             }
             if (dump && li < ncand) {                                    // states after the tile stopped: NaN
@@ -487,8 +489,8 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     }
                 }
                 bool push = false;
-                if (MODE == MODE_TICK && verify) {                       // near the boundary: the FP32 kernel decides (warp-aggregated append)
-                    push = valid && near;
+                if (verify) {                                            // near the boundary: the FP32 kernel decides (warp-aggregated append)
+                    push = li < ncand && inputs_ok && near;
                     // kRecheckBuckets lists by the first pass's step count, longest first: the second pass then walks candidates
                     // of similar life time together (its warps stop together, its long CTAs start first)
                     const int bucket = kRecheckBuckets - 1 - min(kRecheckBuckets - 1, steps * kRecheckBuckets / H);
@@ -540,7 +542,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     }
     // ---- a6 + a7
     block_select_and_finalise<kTcStateWarps + 1>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, a.work,
-                                                  (D == 32) && a.recheck != nullptr);
+                                                  a.recheck != nullptr);
 }
 
 }  // namespace mpmi

@@ -72,7 +72,12 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
     const float *kp = sK + rg * 4;                // rows  q*(4 RG) + rg*4 + e,  q < QR
     const float *zp = zw + cg * 4;                // cands q*(4 CG) + cg*4 + e,  q < 2
     const int col = lane % WC;                    // the candidate this lane fills and tests (lanes >= WC mirror)
-    const long long nbatch = (ncand + WC - 1) / WC;
+    // second pass of the verified tensor-core tick / batch (kernel_args.cuh): walk the deferral lists, longest-lived first
+    const bool rc = a.recheck_mode != 0;
+    int rc_count[kRecheckBuckets], rc_total = 0;
+#pragma unroll
+    for (int b = 0; b < kRecheckBuckets; b++) { rc_count[b] = rc ? (int)a.recheck_count[b] : 0; rc_total += rc_count[b]; }
+    const long long nbatch = ((rc ? (long long)rc_total : ncand) + WC - 1) / WC;
 
     unsigned long long key = kKeyNone;
     unsigned n_safe = 0, n_exec = 0;
@@ -90,6 +95,16 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
         const long long wbatch = (MODE == MODE_TICK && a.perm) ? (batch == 0 ? nbatch - 1 : batch - 1) : batch;
         long long li = wbatch * WC + col;
         if (MODE == MODE_TICK && a.perm && li < a.nsamp) li = a.perm[li];
+        if (rc) {                                          // slot li of the concatenated lists -> candidate
+            int p = (int)li;
+            long long hit = ncand;
+#pragma unroll
+            for (int b = 0; b < kRecheckBuckets; b++) {
+                if (p >= 0 && p < rc_count[b]) hit = (long long)a.recheck[(long long)b * ncand + p];
+                p -= rc_count[b];                          // negative once the slot has been found
+            }
+            li = hit;
+        }
         bool alive = li < ncand && inputs_ok;
         int steps = 0;
         {
@@ -222,12 +237,17 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
         __syncthreads();
         if (tid == 0) {
             __threadfence();
-            if (atomicAdd(&a.st->ticket, 1u) == gridDim.x - 1) { *a.work = 0u; a.st->ticket = 0u; __threadfence(); }
+            if (atomicAdd(&a.st->ticket, 1u) == gridDim.x - 1) {
+                *a.work = 0u; a.st->ticket = 0u;
+                if (rc) for (int b = 0; b < kRecheckBuckets; b++) a.recheck_count[b] = 0u;
+                __threadfence();
+            }
         }
         return;
     }
     // ---- a6 + a7
-    block_select_and_finalise<kTileWarps>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, a.work);
+    block_select_and_finalise<kTileWarps>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, a.work, false,
+                                          rc ? a.recheck_count : nullptr, kRecheckBuckets, a.deferred_out);
 }
 
 }  // namespace mpmi

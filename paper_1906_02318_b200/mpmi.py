@@ -16,7 +16,7 @@ DUMP_NONE, DUMP_PHYS, DUMP_LIFTED = 0, 1, 2
 OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4
 VARIANT_NARROW, VARIANT_WIDE, VARIANT_NO_BINNING, VARIANT_FORCE_BINNING, VARIANT_LATENCY = 1, 2, 4, 8, 16
 VARIANT_LAT_R2, VARIANT_LAT_R4, VARIANT_NO_TENSOR, VARIANT_AFFINE, VARIANT_NO_PREDICT = 32, 64, 128, 256, 512
-VARIANT_TENSOR32, VARIANT_SMEM_MODEL = 1024, 2048
+VARIANT_TENSOR32, VARIANT_SMEM_MODEL, VARIANT_TC_UNVERIFIED = 1024, 2048, 4096
 
 EXPORTS = ("mpmi_create", "mpmi_destroy", "mpmi_step", "mpmi_step_result", "mpmi_step_sync",
            "mpmi_step_device", "mpmi_step_trace", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",

@@ -200,3 +200,130 @@ def test_affine_and_tensor32_flags_together(mp):
         if (ref["margin_all"] > MARGIN).all():
             assert (a["index"], a["safe"], a["steps"], a["n_safe"], a["n_exec"]) == (b["index"], b["safe"], b["steps"], b["n_safe"], b["n_exec"])
         compare_tick(mp, both, o, w, x0, uu, t)
+
+
+# ------------------------------------------------------------------ verified tensor-core tick == FP32 tick -----------
+def _steps_of(mp, ctx, w, x0, uu, t):
+    r, st = trace_tick(mp, ctx, w, x0, uu, t)
+    return r, st
+
+
+def _c4_off_origin(cx, H, gain):
+    """C4's race-car model on an annular track centred far from the origin: states |x| ~ cx + 11.5 and lifted
+    features up to |x|^2 against a 4-wide track, so tau must follow the state scale, not the size of the bounds.  K contracts
+    toward the origin, hence the short horizon; S is the oracle's lift at the shifted nominal state (as oracle/calibrate.py
+    does for C3 / C4), the input gain is raised so that the candidate set is mixed."""
+    w0 = W.make("C4")
+    xn = w0.x_nom.copy(); xn[0] += cx
+    S = np.maximum(np.abs(_oracle(w0, N=1).lift(xn.astype(np.float64))), 1.0)
+    w = W.make("C4", N=1 << 18, H=H, S=S, gamma=w0.gamma * gain)
+    w.cx = cx; w.x_nom = xn
+    return w
+
+
+def _verified_cases():
+    return {
+        "C4_full": W.make("C4"),
+        "C5_full": W.make("C5"),
+        "C5_x100": G.rescaled_units(W.make("C5", N=1 << 17), 100.0),
+        "C5_x1000": G.rescaled_units(W.make("C5", N=1 << 17), 1000.0),
+        "C4_off_origin_30": _c4_off_origin(30.0, 20, 3.0),
+        "C4_off_origin_100": _c4_off_origin(100.0, 12, 10.0),
+        "C4_noise": W.make("C4", N=1 << 18),
+        "C5_noise": W.make("C5", N=1 << 16),
+    }
+
+
+@pytest.mark.parametrize("case", ["C4_full", "C5_full", "C5_x100", "C5_x1000", "C4_off_origin_30", "C4_off_origin_100", "C4_noise", "C5_noise"])
+def test_verified_tick_equals_fp32_tick_every_candidate(mp, case):
+    """The verified tensor-core tick (default at padded d = 128, and at d = 32 from 2^17 candidates) must reproduce the FP32
+    tick candidate by candidate: every step count, hence every flag, and the winner --
+    at the sizes bench.py times, with the state scaled up 100x and 1000x against the absolute margin, with the annulus far
+    from the origin, and with prediction noise.  The second pass must stay a small fraction of the candidates."""
+    V = mp.mpmi
+    w = _verified_cases()[case]
+    if case.endswith("noise"):
+        w.noise_sigma = 0.01
+    ver = mp.Context(w)
+    fp32 = mp.Context(w, variant=V.VARIANT_NO_TENSOR)
+    assert ver.info()["variant"] == 4 and fp32.info()["variant"] in (1, 2)
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    fracs = []
+    for x0, uu, t in zip(x0s, uus, ticks):
+        rv, sv = trace_tick(mp, ver, w, x0, uu, t)
+        rf, sf = trace_tick(mp, fp32, w, x0, uu, t)
+        diff = np.nonzero(sv != sf)[0]
+        assert len(diff) == 0, (case, len(diff), diff[:5], sv[diff[:5]], sf[diff[:5]])
+        assert (rv["index"], rv["safe"], rv["steps"], rv["n_safe"], rv["n_exec"], rv["key"]) == \
+               (rf["index"], rf["safe"], rf["steps"], rf["n_safe"], rf["n_exec"], rf["key"])
+        assert np.array_equal(rv["u"], rf["u"]) and rv["dist"] == rf["dist"]
+        assert 0.05 < (sf == w.H).mean() < 0.95                              # a mixed candidate set
+        ver.step_sync(x0, uu, int(t))
+        fracs.append(ver.info()["reserved"] / (w.N + 1))
+    assert 0 < min(fracs) and max(fracs) < 0.35, fracs
+    print(f"{case}: second pass rolled {min(fracs):.4f} .. {max(fracs):.4f} of the candidates")
+
+
+def test_bare_tensor_core_rollout_breaks_where_the_verified_tick_holds(mp):
+    """Why the tick is verified: at |z| ~ 1e2 (C4) the bare 3xTF32 rollout (MPMI_VARIANT_TC_UNVERIFIED) decides some
+    candidates differently from the FP32 rollout, the verified tick none."""
+    V = mp.mpmi
+    w = W.make("C4", N=1 << 19)
+    bare = mp.Context(w, variant=V.VARIANT_TC_UNVERIFIED)
+    ver = mp.Context(w)
+    fp32 = mp.Context(w, variant=V.VARIANT_NO_TENSOR)
+    assert bare.info()["variant"] == 4 and bare.info()["launches_per_tick"] == 3 and ver.info()["launches_per_tick"] == 6
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    nbare = 0
+    for x0, uu, t in zip(x0s, uus, ticks):
+        _, sb = trace_tick(mp, bare, w, x0, uu, t)
+        _, sv = trace_tick(mp, ver, w, x0, uu, t)
+        _, sf = trace_tick(mp, fp32, w, x0, uu, t)
+        nbare += int((sb != sf).sum())
+        assert np.array_equal(sv, sf)
+        assert np.abs(sb - sf).max() <= 1                                    # (the bare kernel is off by one step where it differs)
+    assert nbare > 0, "the bare kernel agreed everywhere: this workload no longer shows why the tick is verified"
+    print(f"bare tensor-core rollout: {nbare} of {3 * (w.N + 1)} step counts differ from the FP32 rollout; verified tick: 0")
+
+
+@pytest.mark.parametrize("name,kernel", [("C4", "tc"), ("C4", "fp32"), ("C5", "tc"), ("C5", "fp32"), ("T48", "fp32")])
+def test_single_step_error_within_bound(mp, name, kernel):
+    """The per-step constants of csrc/bound.cuh, measured: one rollout step z_2 = K z_1 + B u of every kernel against the exact
+    (FP64) product of the SAME fp32 z_1, row by row, must stay inside E_r = sum_c w_c |K_rc| |z_1c| with
+      FP32 kernels:   w_c = 2^-24 (D + M - c)                                   (sequential FMA chain, column order)
+      tcgen05 kernel: w_c = 2^-19 + 2^-22 (KB + 1 - blk(c)) + 2^-31 (2 KB + 3)   (3xTF32 operands + <= 2 ulp per MMA).
+    (Internal column order = the caller's for these workloads: the constrained dims already come first.)"""
+    V = mp.mpmi
+    N = 4096
+    w = G.scaled_bounds(W.make(name, N=N), 1000.0)                           # nothing leaves the safe set: two full steps each
+    var = {"tc": V.VARIANT_TC_UNVERIFIED | V.VARIANT_TENSOR32, "fp32": V.VARIANT_NO_TENSOR | V.VARIANT_NARROW}[kernel]
+    ctx = mp.Context(w, variant=var)
+    D = ctx.info()["d_pad"]
+    assert ctx.info()["variant"] == (4 if kernel == "tc" else (1 if D <= 32 else 2))
+    rng = np.random.default_rng(7)
+    U = rng.uniform(w.u_lo, w.u_hi, (N, w.m)).astype(np.float32)
+    x0s, _, _ = W.tick_inputs(w, N)
+    x0s = (w.x_nom[None, :] + 3.0 * (x0s - w.x_nom[None, :])).astype(np.float32)   # a wider spread of states
+    traj = torch.full((2, w.d, N), 7.0, dtype=torch.float32, device="cuda")
+    steps = torch.empty(N, dtype=torch.int32, device="cuda")
+    dU, dX = _dev(U), _dev(x0s)
+    ctx.rollout_batch(dU.data_ptr(), dX.data_ptr(), N, N, 2, mp.DUMP_LIFTED, traj.data_ptr(), steps.data_ptr(), 0)
+    torch.cuda.synchronize()
+    assert int(steps.min().item()) == 2
+    z = traj.cpu().numpy().astype(np.float64)                                # (2, d, N)
+    z1, z2 = z[0].T, z[1].T                                                  # (N, d)
+    K = w.K.astype(np.float64); B = w.B.astype(np.float64)
+    exact = z1 @ K.T + U.astype(np.float64) @ B.T
+    aug = np.concatenate([np.abs(z1), np.abs(U.astype(np.float64))], axis=1)                       # (N, d + m) in chain order ...
+    Kaug = np.concatenate([np.abs(K), np.abs(B)], axis=1)                                          # ... state columns, then input
+    M, KB = w.m, D // 8
+    col = np.concatenate([np.arange(w.d), D + np.arange(M)])                                       # position of each column in the padded chain
+    if kernel == "fp32":
+        wc = 2.0 ** -24 * (D + M - col)
+    else:
+        blk = np.where(col < D, col // 8, KB)
+        wc = 2.0 ** -19 + 2.0 ** -22 * (KB + 1 - blk) + 2.0 ** -31 * (2 * KB + 3)
+    E = aug @ (Kaug * wc[None, :]).T                                         # (N, d)
+    ratio = np.abs(z2 - exact) / np.maximum(E, 1e-300)
+    print(f"{name} {kernel}: worst |error| / bound = {ratio.max():.3f}, median {np.median(ratio):.4f}")
+    assert ratio.max() <= 1.0, ratio.max()

@@ -183,6 +183,20 @@ def scaled_bounds(w, factor):
     return v
 
 
+def rescaled_units(w, s):
+    """The same RFF workload (C5, T48) with the physical state measured in units s times smaller, x -> s x: lifted states,
+    bounds and input gain grow by s while every trajectory is the same up to that factor -- the stress case in which the
+    ABSOLUTE 1e-4 margin of rule T2 becomes relative 1e-4 / s."""
+    import copy
+    assert w.lift_kind == 1
+    v = copy.copy(w)
+    v.W = (w.W / s).astype(np.float32); v.scale = float(np.float32(w.scale * s))
+    v.B = (w.B * s).astype(np.float32)
+    v.blo = (w.blo * s).astype(np.float32); v.bhi = (w.bhi * s).astype(np.float32)
+    v.x_nom = (w.x_nom * s).astype(np.float32); v.x_pert = (w.x_pert * s).astype(np.float32)
+    return v
+
+
 def tick_inputs(w, count, seed=None):
     """(x0_t, u_user_t, tick_t) for t < count: x0 = x_nom + seeded perturbation,
     u_user uniform in a box 10 % wider than the input box (so clamping is exercised)."""
