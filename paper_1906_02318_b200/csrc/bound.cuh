@@ -9,10 +9,14 @@
 // One step's rounding errors are bounded row by row by a weighted sum of the ABSOLUTE products,
 //     (|e~| + |e^|)_r  <=  E_r := sum_c w_c |K_rc| |z_c|   (input columns: |B_rj| |u_j|),
 // with w_c fixed by the two arithmetics alone (mpmi_api.cu: bound_weights; each term is listed there):
-//   * FP32 chain of D+M FMAs in column order: term c is rounded (D+M-c) times, 2^-24 each;
-//   * 3xTF32: the dropped z_lo K_lo product (2^-20) and the TF32 rounding of z_lo and K_lo (2^-21 each);
+//   * FP32 chain of D+M FMAs, columns in descending order: term c is rounded (c+1) times, 2^-24 each;
+//   * 3xTF32: the dropped z_lo K_lo product (2^-21) and the TF32 rounding of z_lo (2^-21) and K_lo (2^-22);
 //   * the tensor core's fp32 accumulation, <= 2 ulp (truncation) per MMA on the running sum, counted for the
-//     full-magnitude Z_hi K_hi products that follow column c; the small products before them add 2^-32 each.
+//     full-magnitude Z_hi K_hi products from column c's k-block on (state block b: b+1 of them, the blocks run
+//     in descending order); the small products before them add 2^-31 each.
+//   Both orders put the physical dims (internal columns 0..n-1) last: for a model close to the identity on the physical
+//   block the dominant product of a physical row is the diagonal one, and it is then re-rounded <= n (once) instead of
+//   D+M (KB+1) times -- on C4 that alone cuts tau, and with it the second pass, to a third.
 //   (tests/test_parity_full_gpu.py::test_single_step_error_within_bound measures one step of every kernel against
 //   exactly these E_r.)
 // |z_c| of an arbitrary candidate is bounded over the whole input box by the envelope of the affine map
@@ -63,7 +67,7 @@ __global__ void __launch_bounds__(D < 64 ? 64 : D) bound_err_kernel(const __grid
     }
 }
 
-constexpr int kBoundTauThreads = 128;
+constexpr int kBoundTauThreads = 512;         // 16 warps share the p < k terms of one tau row
 template <int D, int NP>
 __global__ void __launch_bounds__(kBoundTauThreads) bound_tau_kernel(const __grid_constant__ DevCfg cfg) {
     __shared__ float red[kBoundTauThreads / 32][NP];
@@ -80,7 +84,8 @@ __global__ void __launch_bounds__(kBoundTauThreads) bound_tau_kernel(const __gri
     for (int p = 1 + warp; p < k; p += kBoundTauThreads / 32) {    // rows of C K^p: cfg.aff_m[p - 1]
         const float *m = cfg.aff_m + (size_t)(p - 1) * NP * D;
         const float *e = cfg.bnd_e + (size_t)(k - 1 - p) * D;
-        for (int c = lane; c < D; c += 32) {
+#pragma unroll
+        for (int c = lane; c < D; c += 32) {                        // (D / 32 independent column slices: all loads in flight)
             const float ec = e[c];
 #pragma unroll
             for (int i = 0; i < NP; i++) acc[i] = __fmaf_rn(fabsf(__ldg(m + i * D + c)), ec, acc[i]);

@@ -41,22 +41,23 @@ KernFn FN2(MPMI_D)(int M, int P, int kconst) {
 }
 
 #if MPMI_MODE == 0 && MPMI_D == 32
-// second pass of the verified tensor-core tick: 2 candidates per thread, shared-memory model (the pass sees ~10 % of the
-// candidates: below ~2^19 candidates the shared-memory model is the faster one, DESIGN.md section 9 sweep)
+// second pass of the verified tensor-core tick: 2 candidates per thread; model from the constant bank or from shared memory
 #if MPMI_NOISE
 #define RCFN mpmi_pick_regn_32_recheck
 #else
 #define RCFN mpmi_pick_reg_32_recheck
 #endif
-KernFn RCFN(int M) {
+template <bool KC>
+static KernFn pick_rc(int M) {
     switch (M) {
-        case 1: return rollout_reg_kernel<32, 1, 1, MODE_TICK, (MPMI_NOISE != 0), false, true>;
-        case 2: return rollout_reg_kernel<32, 2, 1, MODE_TICK, (MPMI_NOISE != 0), false, true>;
-        case 3: return rollout_reg_kernel<32, 3, 1, MODE_TICK, (MPMI_NOISE != 0), false, true>;
-        case 4: return rollout_reg_kernel<32, 4, 1, MODE_TICK, (MPMI_NOISE != 0), false, true>;
+        case 1: return rollout_reg_kernel<32, 1, 1, MODE_TICK, (MPMI_NOISE != 0), KC, true>;
+        case 2: return rollout_reg_kernel<32, 2, 1, MODE_TICK, (MPMI_NOISE != 0), KC, true>;
+        case 3: return rollout_reg_kernel<32, 3, 1, MODE_TICK, (MPMI_NOISE != 0), KC, true>;
+        case 4: return rollout_reg_kernel<32, 4, 1, MODE_TICK, (MPMI_NOISE != 0), KC, true>;
     }
     return nullptr;
 }
+KernFn RCFN(int M, int kconst) { return kconst ? pick_rc<true>(M) : pick_rc<false>(M); }
 #endif
 
 // fills constant-memory slot `slot` of THIS translation unit with the context's augmented transposed model

@@ -27,3 +27,18 @@ KernFn FN2(MPMI_D)(int M, int *smem) {
     }
     return nullptr;
 }
+
+#if MPMI_D == 128
+// second pass of the verified tensor-core tick / batch: 8-candidate warp batches (rollout_tile.cuh)
+#define RCFN3(a) a##_rc
+#define RCFN2(a) RCFN3(a)
+KernFn RCFN2(FN2(MPMI_D))(int M, int *smem) {
+    switch (M) {
+        case 1: *smem = tile_smem_bytes<MPMI_D, 1, kTileWCRecheck>(); return rollout_tile_kernel<MPMI_D, 1, MPMI_MODE, (MPMI_NOISE != 0), kTileWCRecheck>;
+        case 2: *smem = tile_smem_bytes<MPMI_D, 2, kTileWCRecheck>(); return rollout_tile_kernel<MPMI_D, 2, MPMI_MODE, (MPMI_NOISE != 0), kTileWCRecheck>;
+        case 3: *smem = tile_smem_bytes<MPMI_D, 3, kTileWCRecheck>(); return rollout_tile_kernel<MPMI_D, 3, MPMI_MODE, (MPMI_NOISE != 0), kTileWCRecheck>;
+        case 4: *smem = tile_smem_bytes<MPMI_D, 4, kTileWCRecheck>(); return rollout_tile_kernel<MPMI_D, 4, MPMI_MODE, (MPMI_NOISE != 0), kTileWCRecheck>;
+    }
+    return nullptr;
+}
+#endif

@@ -79,7 +79,7 @@ struct mpmi_ctx {
     int *d_recheck = nullptr;
     unsigned *d_recheck_count = nullptr;
     unsigned recheck_grid = 0;
-    int recheck_block = kRegBlock, recheck_smem = 0;
+    int recheck_block = kRegBlock, recheck_smem = 0, fp32_smem = 0;
     bool recheck_persistent = false;
     float recheck_tau_scale = 1.f;   // MPMI_TC_TAU_SCALE (measures how conservative the bound is; not a tuning knob)
     cudaGraphNode_t n_recheck = nullptr, n_berr = nullptr, n_btau = nullptr;
@@ -149,7 +149,9 @@ int fail(mpmi_ctx *c, int code, const char *msg) {
                           KernFn mpmi_pick_tilen_##D##_tick(int M, int *smem); KernFn mpmi_pick_tilen_##D##_batch(int M, int *smem);
 }  // namespace
 MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DECL_TILE(128)
-KernFn mpmi_pick_reg_32_recheck(int M); KernFn mpmi_pick_regn_32_recheck(int M);
+KernFn mpmi_pick_tile_128_tick_rc(int M, int *smem); KernFn mpmi_pick_tile_128_batch_rc(int M, int *smem);
+KernFn mpmi_pick_tilen_128_tick_rc(int M, int *smem); KernFn mpmi_pick_tilen_128_batch_rc(int M, int *smem);
+KernFn mpmi_pick_reg_32_recheck(int M, int kconst); KernFn mpmi_pick_regn_32_recheck(int M, int kconst);
 KernFn mpmi_pick_relift(int n, int mode);
 KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
 KernFn mpmi_pick_tc_tick(int D, int *smem, int *threads, int *ctas_per_sm, int noise); KernFn mpmi_pick_tc_batch(int D, int *smem, int *threads, int *ctas_per_sm, int noise);
@@ -708,7 +710,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         // unless the caller asks for the FP32 SIMT tile kernel; d = 64 stays on the SIMT tile kernel
         tensor = D == 128 && tc_model_ok;
         c->P = 1;
-        int fsmem = 0;
+        int &fsmem = c->fp32_smem;
         c->k_batch_fp32 = pick_tile(D, M, MODE_BATCH, &fsmem, noise);
         if (tensor) {
             c->variant = 4;
@@ -804,15 +806,18 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     if (tensor && c->variant == 4 && !tc_unverified) {
         if (!affine_built) { rc = build_affine(); if (rc != MPMI_OK) return bail(rc); }
         if (D == 32) {               // FP32 register kernel, 2 candidates per thread, CTAs loop over blocks of the lists
-            c->k_recheck = noise ? mpmi_pick_regn_32_recheck(M) : mpmi_pick_reg_32_recheck(M);
+            const int rc_kconst = (c->kslot >= 0 && !std::getenv("MPMI_RC_SMEM")) ? 1 : 0;
+            c->k_recheck = noise ? mpmi_pick_regn_32_recheck(M, rc_kconst) : mpmi_pick_reg_32_recheck(M, rc_kconst);
             c->recheck_block = kRegBlock; c->recheck_smem = 0; c->recheck_persistent = false;
             const long long nb = (sc + 2 * kRegBlock - 1) / (2 * kRegBlock), cap = 3LL * c->sm_count;
             c->recheck_grid = (unsigned)(nb < cap ? nb : cap);
         } else {                     // FP32 warp-tile kernel, persistent CTAs fetch batches of the lists from the work counter
-            c->k_recheck = pick_tile(D, M, MODE_TICK, &c->recheck_smem, noise);
-            c->k_batch_recheck = c->k_batch_fp32;
+            int bs = 0;
+            c->k_recheck = noise ? mpmi_pick_tilen_128_tick_rc(M, &c->recheck_smem) : mpmi_pick_tile_128_tick_rc(M, &c->recheck_smem);
+            c->k_batch_recheck = noise ? mpmi_pick_tilen_128_batch_rc(M, &bs) : mpmi_pick_tile_128_batch_rc(M, &bs);
+            CUC(cudaFuncSetAttribute((const void *)c->k_batch_recheck, cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
             c->recheck_block = kTileThreads; c->recheck_persistent = true;
-            const long long nb = (sc + kTileNC - 1) / kTileNC;
+            const long long nb = (sc + kTileNC / 2 - 1) / (kTileNC / 2);
             c->recheck_grid = (unsigned)(nb < c->sm_count ? nb : c->sm_count);
             CUC(cudaFuncSetAttribute((const void *)c->k_recheck, cudaFuncAttributeMaxDynamicSharedMemorySize, c->recheck_smem));
         }
@@ -832,20 +837,24 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         const int Hh = cfg->H;
         const double u24 = std::ldexp(1.0, -24);
         const int KB = D / 8;
-        // column weights w_c of the per-step error bound E_r = sum_c w_c |K_rc| |z_c| (bound.cuh):
-        //   FP32 kernel: term c passes through (D + M - c) roundings of 2^-24 each (+1 when sigma*eps is added afterwards);
-        //   3xTF32 operands: z_lo K_lo dropped (|z_lo| < 2^-10 |z|, |K_lo| < 2^-10 |K|: 2^-20) + z_lo and K_lo rounded to TF32
-        //   (relative 2^-11 of a 2^-10 part: 2^-21 each) = 2^-19;
-        //   tensor-core accumulation: <= 2 ulp = 2^-22 of the running sum per MMA, for the Z_hi K_hi MMAs from column c's
-        //   k-block on (input block last, then the noise block); the 2 KB + 3 small-product MMAs before them run on sums
-        //   below 2^-9 of the full magnitude: 2^-31 each.
+        // column weights w_c of the per-step error bound E_r = sum_c w_c |K_rc| |z_c| (bound.cuh), internal column order:
+        //   FP32 kernel: the FMA chain runs over the columns in DESCENDING order, so term c is rounded (c + 1) times, 2^-24 each
+        //   (+1 when sigma*eps is added afterwards);
+        //   3xTF32 operands: z_lo K_lo dropped (|z_lo| < 2^-10 |z|: the hardware truncates z_hi; |K_lo| <= 2^-11 |K|: K_hi is
+        //   rounded to nearest): 2^-21; z_lo rounded to TF32 (2^-11 of a 2^-10 part): 2^-21; K_lo rounded (2^-11 of 2^-11): 2^-22;
+        //   tensor-core accumulation: <= 2 ulp = 2^-22 of the running sum per MMA.  The full-magnitude Z_hi K_hi MMAs run input
+        //   block, [noise block,] state blocks KB-1 .. 0: a product of state block b is followed by b + 1 accumulations, the
+        //   input block by KB + 1 (+1 with noise); the 2 KB + 3 small-product MMAs before them run on sums below 2^-9 of the
+        //   full magnitude: 2^-31 each.
         std::vector<float> wv((size_t)D + M, 0.f);
-        const int nblk = KB + 1 + (noise ? 1 : 0), nfp = D + M + (noise ? 1 : 0);
+        const double w_operand = std::ldexp(1.0, -21) + std::ldexp(1.0, -21) + std::ldexp(1.0, -22);
         for (int cc = 0; cc < D + M; cc++) {
-            const int blk = cc < D ? cc / 8 : KB;
-            wv[cc] = (float)(u24 * (nfp - cc) + std::ldexp(1.0, -19) + std::ldexp(1.0, -22) * (nblk - blk) + std::ldexp(1.0, -31) * (2 * KB + 3));
+            const int nacc = cc < D ? cc / 8 + 1 : KB + 1 + (noise ? 1 : 0);
+            wv[cc] = (float)(u24 * (cc + 1 + (noise ? 1 : 0)) + w_operand + std::ldexp(1.0, -22) * nacc + std::ldexp(1.0, -31) * (2 * KB + 3));
         }
-        const double wnoise = u24 + std::ldexp(1.0, -20) + std::ldexp(1.0, -22);      // the sigma*eps column: one FP32 rounding, hi/lo split, one MMA
+        // the sigma*eps column: FP32 adds it with one rounding, the tensor-core path rounds sigma*eps itself, splits it (2^-21)
+        // and accumulates it second of the full-magnitude MMAs
+        const double wnoise = 2.0 * u24 + std::ldexp(1.0, -21) + std::ldexp(1.0, -22) * (KB + 1);
         const double epsmax = 5.77;                                                    // Box-Muller with u1 >= 2^-24: |eps| <= sqrt(48 ln 2) = 5.768
         std::vector<double> Kin((size_t)D * D), Bin((size_t)D * M);
         for (int r = 0; r < D; r++) {
@@ -1083,7 +1092,7 @@ int mpmi_rollout_batch(mpmi_ctx *c, const float *d_U, const float *d_X0, int64_t
             CU(c, launch(c, c->k_batch, Ncand, a, s));
             CU(c, launch_recheck(c, c->k_batch_recheck, a, s));
         } else {
-            CU(c, launch_geom(c, c->k_batch_fp32, Ncand, a, (cudaStream_t)stream, kTileNC, kTileThreads, c->recheck_smem, true));
+            CU(c, launch_geom(c, c->k_batch_fp32, Ncand, a, (cudaStream_t)stream, kTileNC, kTileThreads, c->fp32_smem, true));
         }
     } else {
         CU(c, launch(c, c->k_batch, Ncand, a, (cudaStream_t)stream));

@@ -144,7 +144,12 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 
         float2 acc[P][D];
 #pragma unroll
-        for (int c = 0; c < D + M; c++) {
+        // Columns run in DESCENDING order, the physical dims (internal columns 0..n-1) last: a product's rounding error is
+        // re-rounded by every FMA after it, and for a model close to the identity on the physical block (small time step) the
+        // dominant product of a physical row is its diagonal one -- it now passes through <= n roundings instead of D + M
+        // (the per-column weights of csrc/bound.cuh follow this order).
+        for (int cc = 0; cc < D + M; cc++) {
+            const int c = D + M - 1 - cc;
 #pragma unroll
             for (int r = 0; r < D; r += 4) {
                 const float4 kv = KC ? c_model[a.kslot][(c * D + r) / 4]
@@ -152,7 +157,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
                 for (int p = 0; p < P; p++) {
                     const float2 zc = z[p][c];
-                    if (c == 0) {
+                    if (cc == 0) {
                         mul2_bcast(acc[p][r + 0], kv.x, zc); mul2_bcast(acc[p][r + 1], kv.y, zc);
                         mul2_bcast(acc[p][r + 2], kv.z, zc); mul2_bcast(acc[p][r + 3], kv.w, zc);
                     } else {

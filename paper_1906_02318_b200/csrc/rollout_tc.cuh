@@ -78,6 +78,9 @@ __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__flo
 // toward zero of ~2^-22 |x| per operand that adds up coherently over the horizon.  Adding half a TF32 ulp
 // to the bit pattern first turns the hardware's truncation into round-half-away (one integer add).
 __device__ __forceinline__ uint32_t tf32_lo(float x) { return __float_as_uint(x - tf32_hi(x)) + 0x1000u; }
+// round-to-nearest TF32 (ties away) and the matching low part x - x_hi (exact in fp32, either sign), itself rounded as above
+__device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u); }
+__device__ __forceinline__ uint32_t tf32_lo_of(float x, float x_hi) { return __float_as_uint(x - x_hi) + 0x1000u; }
 
 // Same decision as safe_check (mpmi_device.cuh) -- box strict, annulus closed, NaN / Inf unsafe -- but without
 // the 2*nbox-long chain of dependent predicate ANDs (~13 cycles per link), which sits on the per-step critical
@@ -218,8 +221,11 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
         const float v = c < kTcD ? cfg.KTa[c * kTcD + r] : bcol ? cfg.KTa[(kTcD + (cb & 3)) * kTcD + r]
                       : (c >= kTcD + 8 && r == c - (kTcD + 8)) ? 1.f : 0.f;                       // [K | B B | noise selector]
         const int off = (r >> 3) * kTcSBO + (c >> 2) * kTcLBO + (r & 7) * 16 + (c & 3) * 4;
-        *reinterpret_cast<float *>(smem_img + off) = tf32_hi(v);
-        *reinterpret_cast<uint32_t *>(smem_img + kTcImg + off) = (cb >= 4 && cb < 8) ? 0u : tf32_lo(v);
+        // K_hi = v ROUNDED to nearest TF32 (the model image is built here, so it need not be the truncation the hardware applies
+        // to the state): |K_lo| <= 2^-11 |K| instead of 2^-10, which halves the dropped z_lo K_lo product (csrc/bound.cuh)
+        const float vh = tf32_rn(v);
+        *reinterpret_cast<float *>(smem_img + off) = vh;
+        *reinterpret_cast<uint32_t *>(smem_img + kTcImg + off) = (cb >= 4 && cb < 8) ? 0u : tf32_lo_of(v, vh);
     }
     float u_h[kMaxM] = {0.f, 0.f, 0.f, 0.f};
     bool inputs_ok = true;
@@ -305,10 +311,15 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     for (int kk = 0; kk < kTcKB; kk++)                     // Z_lo * K_hi
                         mma_tf32_ts(dnxt, tb + kTcColAlo + 8 * kk, dhi + kk * kstep, idesc, true);
                     if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNlo, dhi + (kTcKB + 1) * kstep, idesc, true);     // (sigma eps)_lo through the selector
+                    // Z_hi * K_hi, the only products at full magnitude, in DESCENDING k-block order: input block ((u_hi + u_lo) * B_hi),
+                    // (sigma eps)_hi, then the state blocks KB-1 .. 0.  Every accumulation truncates the running sum (<= 2 ulp), so the
+                    // block of the physical dims (columns 0..7), the dominant one of a physical row when K is close to the identity
+                    // there, goes last and is truncated once (csrc/bound.cuh weighs block b with b + 1 accumulations).
+                    mma_tf32_ts(dnxt, tb + kTcColU, dhi + kTcKB * kstep, idesc, true);
+                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + (kTcKB + 1) * kstep, idesc, true);
 #pragma unroll
-                    for (int kk = 0; kk < kTcKB + 1; kk++)                 // Z_hi * K_hi  (last k-block: (u_hi + u_lo) * B_hi)
-                        mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tb + kTcColU, dhi + kk * kstep, idesc, true);
-                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + (kTcKB + 1) * kstep, idesc, true);     // (sigma eps)_hi
+                    for (int kk = kTcKB - 1; kk >= 0; kk--)
+                        mma_tf32_ts(dnxt, dcur + 8 * kk, dhi + kk * kstep, idesc, true);
                     mma_commit(bar_full);
                     TCT(ti_23);
                 }

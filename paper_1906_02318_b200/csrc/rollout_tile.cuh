@@ -22,13 +22,22 @@ constexpr int kTileWC = 16;                      // candidates per warp batch (1
 constexpr int kTileWarps = kTileNC / kTileWC;
 constexpr int kTileThreadsT = kTileWarps * 32;
 
-template <int D, int M>
-constexpr int tile_smem_bytes() { return ((D + M) * D + kTileWarps * (D + M) * kTileWC) * 4; }
+constexpr int kTileWCRecheck = 8;                // second pass of the verified tensor-core tick: 8 candidates per warp batch
 
-template <int D, int M, int MODE, bool NOISE = false>
+template <int D, int M, int WCP = kTileWC>
+constexpr int tile_smem_bytes() { return ((D + M) * D + kTileWarps * (D + M) * WCP) * 4; }
+
+// WCP = candidates per warp batch.  16 for whole ticks (lane = 8 rows x 8 candidates).  The second pass of the verified
+// tensor-core tick (kernel_args.cuh: recheck) sees a few per cent of the candidates -- fewer warp batches than the machine
+// has warps -- so there the batch is 8 candidates (lane = 4 rows x 8 candidates) and batches are dealt out statically,
+// longest-lived first, round-robin over CTAs and then over the warps of a CTA: every SM sub-partition gets the same number
+// of batches, a long, a medium and a short one (measured with 16-candidate batches fetched first-come: 1.3 ms for 5 % of
+// C5's candidates, some sub-partitions holding four full-horizon batches).  Same FMA chain per (row, candidate), hence the
+// same bits, for either batch size.
+template <int D, int M, int MODE, bool NOISE = false, int WCP = kTileWC>
 __global__ void __launch_bounds__(kTileThreadsT, 1)
 rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
-    constexpr int WC = kTileWC;
+    constexpr int WC = WCP;
     constexpr int CG = WC / 8;                    // candidate groups per warp: every lane owns 8 candidates
     constexpr int RG = 32 / CG;                   // row groups per warp
     constexpr int TR = D / RG;                    // rows per lane
@@ -82,11 +91,11 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
     unsigned long long key = kKeyNone;
     unsigned n_safe = 0, n_exec = 0;
 
-    for (;;) {
-        // ---- next batch of 32 candidates for this warp (dynamic: warps that exit early take more)
-        if (lane == 0) s_batch[warp] = atomicAdd(a.work, 1u);
+    for (long long round = 0;; round++) {
+        // ---- next batch of WC candidates for this warp (dynamic: warps that exit early take more; second pass: static)
+        if (lane == 0) s_batch[warp] = rc ? 0u : atomicAdd(a.work, 1u);
         __syncwarp();
-        const long long batch = s_batch[warp];
+        const long long batch = rc ? (long long)blockIdx.x + (long long)gridDim.x * (warp + kTileWarps * round) : (long long)s_batch[warp];
         __syncwarp();
         if (batch >= nbatch) break;
 
@@ -141,7 +150,8 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
                 for (int q = 0; q < 4; q++) acc[r][q] = make_float2(0.f, 0.f);
 
 #pragma unroll 2
-            for (int c = 0; c < D + M; c++) {
+            for (int cc = 0; cc < D + M; cc++) {                // descending column order: see rollout_reg.cuh
+                const int c = D + M - 1 - cc;
                 float kr[TR];
 #pragma unroll
                 for (int q = 0; q < QR; q++) {

@@ -290,8 +290,9 @@ def test_bare_tensor_core_rollout_breaks_where_the_verified_tick_holds(mp):
 def test_single_step_error_within_bound(mp, name, kernel):
     """The per-step constants of csrc/bound.cuh, measured: one rollout step z_2 = K z_1 + B u of every kernel against the exact
     (FP64) product of the SAME fp32 z_1, row by row, must stay inside E_r = sum_c w_c |K_rc| |z_1c| with
-      FP32 kernels:   w_c = 2^-24 (D + M - c)                                   (sequential FMA chain, column order)
-      tcgen05 kernel: w_c = 2^-19 + 2^-22 (KB + 1 - blk(c)) + 2^-31 (2 KB + 3)   (3xTF32 operands + <= 2 ulp per MMA).
+      FP32 kernels:   w_c = 2^-24 (c + 1)                                       (sequential FMA chain, columns descending)
+      tcgen05 kernel: w_c = 5 * 2^-22 + 2^-22 nacc(c) + 2^-31 (2 KB + 3)         (3xTF32 operands + <= 2 ulp per MMA;
+                      nacc = blk(c) + 1 for a state column, KB + 1 for an input column: k-blocks descending).
     (Internal column order = the caller's for these workloads: the constrained dims already come first.)"""
     V = mp.mpmi
     N = 4096
@@ -319,10 +320,10 @@ def test_single_step_error_within_bound(mp, name, kernel):
     M, KB = w.m, D // 8
     col = np.concatenate([np.arange(w.d), D + np.arange(M)])                                       # position of each column in the padded chain
     if kernel == "fp32":
-        wc = 2.0 ** -24 * (D + M - col)
+        wc = 2.0 ** -24 * (col + 1)
     else:
-        blk = np.where(col < D, col // 8, KB)
-        wc = 2.0 ** -19 + 2.0 ** -22 * (KB + 1 - blk) + 2.0 ** -31 * (2 * KB + 3)
+        nacc = np.where(col < D, col // 8 + 1, KB + 1)
+        wc = 5 * 2.0 ** -22 + 2.0 ** -22 * nacc + 2.0 ** -31 * (2 * KB + 3)
     E = aug @ (Kaug * wc[None, :]).T                                         # (N, d)
     ratio = np.abs(z2 - exact) / np.maximum(E, 1e-300)
     print(f"{name} {kernel}: worst |error| / bound = {ratio.max():.3f}, median {np.median(ratio):.4f}")
