@@ -207,6 +207,14 @@ int mpmi_step_device(mpmi_ctx *ctx, const float *d_x0, const float *d_u_user, ui
 int mpmi_step_trace(mpmi_ctx *ctx, const float *d_x0, const float *d_u_user, uint64_t tick,
                     void *cuda_stream, mpmi_result *d_out, int32_t *d_steps);
 
+/* Measurement aid for bench.py's roofline: while enabled, the plain-launch entries (mpmi_step_device, mpmi_step_trace,
+ * mpmi_shard_step) record CUDA events on cuda_stream before the tick kernel, after it and after the second pass of a
+ * verified tensor-core tick (three event records per tick, no synchronisation).  mpmi_profile_read waits for the
+ * recorded ticks and returns, oldest first, the device time of the tick kernel and of the second pass (0 if there is
+ * none) of the last `*count` <= min(capacity, 64) ticks, in milliseconds (host arrays). */
+int mpmi_profile_enable(mpmi_ctx *ctx, int32_t enable);
+int mpmi_profile_read(mpmi_ctx *ctx, int32_t capacity, int32_t *count, float *ms_tick_kernel, float *ms_second_pass);
+
 /* Sharded tick (section 8(e)): roll out this context's shard and write its mpmi_partial to
  * d_partial (device).  After the caller has gathered the G partials of all ranks into d_partials
  * (device, G entries), mpmi_shard_finalize reduces them (min key, summed counters), regenerates

@@ -90,6 +90,10 @@ struct mpmi_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int *d_deferred_mapped = nullptr;
     KArgs gr{};
+    // mpmi_profile_enable: CUDA events around the tick kernel and the second pass of the plain-launch entries (ring of kProfRing ticks)
+    bool prof = false;
+    std::vector<cudaEvent_t> prof_ev;     // 3 per slot: before the tick kernel, after it, after the second pass
+    unsigned prof_n = 0;
     std::string err;
 };
 
@@ -112,6 +116,7 @@ __global__ void shard_finalise_kernel(const __grid_constant__ DevCfg cfg, const 
 
 namespace {
 
+constexpr unsigned kProfRing = 64;
 constexpr long long kLatMaxCand = 24576;        // <= this many candidates: latency kernel (measured: 125 vs 155 us at 2^14, 210 vs 164 us at 2^15)
 constexpr long long kTc32MinCand = 1LL << 17;   // D = 32: tensor-core kernel from this many candidates (four CTAs per SM need >= 592 tiles to fill)
 
@@ -308,8 +313,12 @@ cudaError_t enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale;
         if (fork) CL(cudaStreamWaitEvent(s, c->ev_join, 0));
     }
+    cudaEvent_t *pe = c->prof ? const_cast<cudaEvent_t *>(&c->prof_ev[3 * (c->prof_n % kProfRing)]) : nullptr;
+    if (pe) CL(cudaEventRecord(pe[0], s));
     CL(launch(c, c->k_tick, c->dc.shard_count, a, s));
+    if (pe) CL(cudaEventRecord(pe[1], s));
     if (c->k_recheck) CL(launch_recheck(c, c->k_recheck, a, s));
+    if (pe) { CL(cudaEventRecord(pe[2], s)); const_cast<mpmi_ctx *>(c)->prof_n++; }
     return cudaSuccess;
 }
 #undef CL
@@ -453,6 +462,7 @@ void mpmi_destroy(mpmi_ctx *c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->side) cudaStreamDestroy(c->side);
+    for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
     cudaFree(c->d_hist); cudaFree(c->d_cursor); cudaFree(c->d_perm); cudaFree(c->d_bin_ticket);
     cudaFreeHost(c->h_res);
     delete c;
@@ -1038,6 +1048,32 @@ int mpmi_step_trace(mpmi_ctx *c, const float *d_x0, const float *d_u_user, uint6
     a.x0 = d_x0; a.u_user = d_u_user; a.tick_val = tick;
     a.st = c->d_state; a.out = d_out; a.steps = d_steps;
     CU(c, enqueue_tick(c, a, (cudaStream_t)stream));
+    return MPMI_OK;
+}
+
+int mpmi_profile_enable(mpmi_ctx *c, int32_t enable) {
+    if (!c) return MPMI_ERR_INVALID;
+    CU(c, cudaSetDevice(c->device));
+    if (enable && c->prof_ev.empty()) {
+        c->prof_ev.resize(3 * kProfRing, nullptr);
+        for (cudaEvent_t &e : c->prof_ev) CU(c, cudaEventCreate(&e));
+    }
+    c->prof = enable != 0; c->prof_n = 0;
+    return MPMI_OK;
+}
+
+int mpmi_profile_read(mpmi_ctx *c, int32_t capacity, int32_t *count, float *ms_tick_kernel, float *ms_second_pass) {
+    if (!c || !count || !ms_tick_kernel || !ms_second_pass || capacity <= 0) return MPMI_ERR_INVALID;
+    CU(c, cudaSetDevice(c->device));
+    const unsigned n = c->prof_n < kProfRing ? c->prof_n : kProfRing;
+    int out = 0;
+    for (unsigned i = c->prof_n - n; i < c->prof_n && out < capacity; i++, out++) {
+        cudaEvent_t *pe = &c->prof_ev[3 * (i % kProfRing)];
+        CU(c, cudaEventSynchronize(pe[2]));
+        CU(c, cudaEventElapsedTime(&ms_tick_kernel[out], pe[0], pe[1]));
+        CU(c, cudaEventElapsedTime(&ms_second_pass[out], pe[1], pe[2]));
+    }
+    *count = out;
     return MPMI_OK;
 }
 

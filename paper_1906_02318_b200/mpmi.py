@@ -19,7 +19,7 @@ VARIANT_LAT_R2, VARIANT_LAT_R4, VARIANT_NO_TENSOR, VARIANT_AFFINE, VARIANT_NO_PR
 VARIANT_TENSOR32, VARIANT_SMEM_MODEL, VARIANT_TC_UNVERIFIED = 1024, 2048, 4096
 
 EXPORTS = ("mpmi_create", "mpmi_destroy", "mpmi_step", "mpmi_step_result", "mpmi_step_sync",
-           "mpmi_step_device", "mpmi_step_trace", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
+           "mpmi_step_device", "mpmi_step_trace", "mpmi_profile_enable", "mpmi_profile_read", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
            "mpmi_get_info", "mpmi_strerror", "mpmi_last_error")
 
 
@@ -100,6 +100,8 @@ def load_library():
     lib.mpmi_step_sync.argtypes = [vp, vp, vp, u64, vp, C.POINTER(Result)]
     lib.mpmi_step_device.argtypes = [vp, vp, vp, u64, vp, vp]
     lib.mpmi_step_trace.argtypes = [vp, vp, vp, u64, vp, vp, vp]
+    lib.mpmi_profile_enable.argtypes = [vp, i32]
+    lib.mpmi_profile_read.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.mpmi_shard_step.argtypes = [vp, vp, vp, u64, vp, vp]
     lib.mpmi_shard_finalize.argtypes = [vp, vp, i32, vp, u64, vp, vp]
     lib.mpmi_rollout_batch.argtypes = [vp, vp, vp, i64, i64, i32, i32, vp, vp, vp, u64, vp]
@@ -210,6 +212,16 @@ class Context:
 
     def step_trace(self, d_x0, d_u_user, tick, stream, d_out, d_steps):
         self._check(self._lib.mpmi_step_trace(self._h, d_x0, d_u_user, int(tick), stream, d_out, d_steps))
+
+    def profile_enable(self, enable=True):
+        self._check(self._lib.mpmi_profile_enable(self._h, 1 if enable else 0))
+
+    def profile_read(self, capacity=64):
+        """(ms of the tick kernel, ms of the second pass) per recorded plain-launch tick, oldest first"""
+        n = C.c_int32(0)
+        a = (C.c_float * capacity)(); b = (C.c_float * capacity)()
+        self._check(self._lib.mpmi_profile_read(self._h, capacity, C.byref(n), a, b))
+        return np.array(a[: n.value], dtype=np.float64), np.array(b[: n.value], dtype=np.float64)
 
     def shard_step(self, d_x0, d_u_user, tick, stream, d_partial):
         self._check(self._lib.mpmi_shard_step(self._h, d_x0, d_u_user, int(tick), stream, d_partial))

@@ -1,6 +1,7 @@
 """GPU parity tests proper: the CUDA path (through the C ABI) against the FP64 oracle, element by
 element on the same seeded inputs.  Run on the B200 box: python -m pytest tests -m gpu."""
 import copy
+import os
 import numpy as np
 import pytest
 
@@ -774,3 +775,52 @@ def test_constant_slot_exhaustion_falls_back_to_shared_memory(mp):
     again = mp.Context(w, variant=NT)                      # a slot is free again
     r = again.step_sync(x0s[0], uus[0], int(ticks[0])).as_dict(w.m)
     assert r["key"] == ref[0]["key"]
+
+
+# ------------------------------------------------------------------ N > 1: two ranks over NCCL (needs 2 GPUs) -------------
+def _nccl_worker(rank, world, port, name, N, nticks, out):
+    import os
+    import torch.distributed as dist
+    import paper_1906_02318_b200 as mpk
+    from paper_1906_02318_b200.shard import shard_plan, gather_partials
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    w = W.make(name, N=N)
+    b, c = shard_plan(w.N, 1, world, rank)
+    ctx = mpk.Context(w, device=rank, shard=(b, c))
+    x0s, uus, ticks = W.tick_inputs(w, nticks)
+    s = torch.cuda.current_stream().cuda_stream
+    part = torch.zeros(3, dtype=torch.int64, device="cuda")
+    res = torch.zeros(56, dtype=torch.uint8, device="cuda")
+    got = []
+    for x0, uu, t in zip(x0s, uus, ticks):
+        dx, du = torch.as_tensor(x0).cuda(), torch.as_tensor(uu).cuda()
+        ctx.shard_step(dx.data_ptr(), du.data_ptr(), int(t), s, part.data_ptr())
+        parts = gather_partials(part, world)
+        ctx.shard_finalize(parts.data_ptr(), world, du.data_ptr(), int(t), s, res.data_ptr())
+        torch.cuda.synchronize()
+        r = np.frombuffer(res.cpu().numpy().tobytes(), dtype=mpk.mpmi.RESULT_DTYPE)[0]
+        got.append((int(r["index"]), int(r["safe"]), int(r["steps"]), int(r["n_safe"]), int(r["n_exec"]), int(r["key"])))
+    out[rank] = got
+    dist.destroy_process_group()
+
+
+def test_two_rank_nccl_sharded_tick(mp):
+    """Candidates sharded over two GPUs, one 24-byte all-gather over NCCL per tick: every rank decodes
+    the result of the single-context tick.  Skipped on a 1-GPU box (the same code path runs there as two shards on one GPU:
+    test_device_and_shard_paths_match_host_path, and through a 1-rank NCCL group: MPMI_BENCH_FORCE_SHARD=1 python bench.py)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 GPUs")
+    import torch.multiprocessing as tmp
+    name, N, nticks = "C4", 1 << 18, 3
+    w = W.make(name, N=N)
+    one = mp.Context(w)
+    x0s, uus, ticks = W.tick_inputs(w, nticks)
+    ref = []
+    for x0, uu, t in zip(x0s, uus, ticks):
+        r = one.step_sync(x0, uu, int(t)).as_dict(w.m)
+        ref.append((r["index"], r["safe"], r["steps"], r["n_safe"], r["n_exec"], r["key"]))
+    out = tmp.Manager().dict()
+    tmp.spawn(_nccl_worker, args=(2, 29500 + os.getpid() % 2000, name, N, nticks, out), nprocs=2, join=True)
+    assert out[0] == ref and out[1] == ref
