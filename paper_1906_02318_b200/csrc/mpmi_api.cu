@@ -818,8 +818,11 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         if (D == 32) {               // FP32 register kernel, 2 candidates per thread, CTAs loop over blocks of the lists
             const int rc_kconst = (c->kslot >= 0 && !std::getenv("MPMI_RC_SMEM")) ? 1 : 0;
             c->k_recheck = noise ? mpmi_pick_regn_32_recheck(M, rc_kconst) : mpmi_pick_reg_32_recheck(M, rc_kconst);
-            c->recheck_block = kRegBlock; c->recheck_smem = 0; c->recheck_persistent = false;
-            const long long nb = (sc + 2 * kRegBlock - 1) / (2 * kRegBlock), cap = 3LL * c->sm_count;
+            // 4 one-warp CTAs per SM (one per sub-partition), each rolling blocks of 64 candidates: its own first, then first come,
+            // first served (rollout_reg.cuh).  Measured on C4 (3.8 % of 2^20 candidates deferred): 4-warp CTAs of 256 candidates
+            // with a static walk 260 us -- the SMs that got two of the long-lived head blocks set the time.
+            c->recheck_block = 32; c->recheck_smem = 0; c->recheck_persistent = false;
+            const long long nb = (sc + 63) / 64, cap = 4LL * c->sm_count;
             c->recheck_grid = (unsigned)(nb < cap ? nb : cap);
         } else {                     // FP32 warp-tile kernel, persistent CTAs fetch batches of the lists from the work counter
             int bs = 0;
@@ -833,8 +836,8 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         }
         if (!c->k_recheck) { c->err = "no second-pass kernel for this (d, m)"; return bail(MPMI_ERR_UNSUPPORTED); }
         CUC(cudaMalloc(&c->d_recheck, sizeof(int) * (size_t)sc * kRecheckBuckets));
-        CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned) * kRecheckBuckets));
-        CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned) * kRecheckBuckets));
+        CUC(cudaMalloc(&c->d_recheck_count, sizeof(unsigned) * (kRecheckBuckets + 1)));       // + the second pass's block counter
+        CUC(cudaMemset(c->d_recheck_count, 0, sizeof(unsigned) * (kRecheckBuckets + 1)));
         if (const char *e = std::getenv("MPMI_TC_TAU_SCALE")) {
             const float v = (float)std::atof(e);
             if (v >= 0.f && v <= 16.f) c->recheck_tau_scale = v;

@@ -287,6 +287,7 @@ __device__ __forceinline__ void block_select_and_finalise(const DevCfg &cfg, uns
             if (lists) {                 // second pass of a verified tick: empty the deferral lists, report how many it rolled
                 unsigned tot = 0;
                 for (int i = 0; i < nlists; i++) { tot += lists[i]; lists[i] = 0u; }
+                lists[nlists] = 0u;      // (the block counter of the second pass, kept behind the list counters)
                 st->pad = tot;
                 if (deferred_out) *reinterpret_cast<volatile int *>(deferred_out) = (int)tot;     // (mapped: before the sequence number)
             }

@@ -27,7 +27,10 @@ constexpr int reg_min_blocks() { return (D * P >= 32) ? 3 : 4; }
 // KC = false: staged in shared memory and read with warp-uniform LDS.128 -- better when an SM holds only one or two
 // warps, which cannot hide the constant-cache misses of a 4.3 KB model (measured crossover: ~2^19 candidates at D = 32).
 // RC = true: second pass of the verified tensor-core tick (kernel_args.cuh): the CTAs walk the deferral lists (longest-lived
-// first) in blocks of 2P * blockDim candidates, block b of CTA x = x + b * gridDim, and the last CTA finalises the tick.
+// first) in blocks of 2P * blockDim candidates.  The pass is launched as 4 one-warp CTAs per SM, one per sub-partition (a
+// warp of FFMA2 saturates its sub-partition's FMA pipe on its own); CTA x starts with block x and fetches every further
+// block from a counter (a.recheck_count[kRecheckBuckets]), so a warp whose candidates stop early takes more, and the
+// long-lived blocks at the head of the lists end up on different sub-partitions.  The last CTA finalises the tick.
 template <int D, int M, int P, int MODE, bool NOISE = false, bool KC = true, bool RC = false>
 __global__ void __launch_bounds__(kRegBlock, reg_min_blocks<D, P>())
 rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
@@ -67,7 +70,7 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     int rc_count[kRecheckBuckets], rc_total = 0;
 #pragma unroll
     for (int b = 0; b < kRecheckBuckets; b++) { rc_count[b] = RC ? (int)a.recheck_count[b] : 0; rc_total += rc_count[b]; }
-  for (long long blk = blockIdx.x; !RC || blk * (2 * P * (long long)blockDim.x) < rc_total; blk += gridDim.x) {
+  for (long long blk = blockIdx.x; !RC || blk * (2 * P * (long long)blockDim.x) < rc_total;) {
     // ---- a1 + a2: candidates of this thread ------------------------------------------------------
     float2 z[P][D + M];
     long long li[S];
@@ -299,6 +302,10 @@ rollout_reg_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         }
     }
     if (!RC) break;
+    // next block of the lists: first come, first served (blockDim == 32: one warp, no block-level hand-off needed)
+    unsigned nxt = 0;
+    if (tid == 0) nxt = atomicAdd(a.recheck_count + kRecheckBuckets, 1u);
+    blk = (long long)gridDim.x + (long long)__shfl_sync(0xffffffffu, nxt, 0);
   }
     block_select_and_finalise<kRegBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq, nullptr, false,
                                               RC ? a.recheck_count : nullptr, kRecheckBuckets, a.deferred_out);

@@ -249,7 +249,7 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
             __threadfence();
             if (atomicAdd(&a.st->ticket, 1u) == gridDim.x - 1) {
                 *a.work = 0u; a.st->ticket = 0u;
-                if (rc) for (int b = 0; b < kRecheckBuckets; b++) a.recheck_count[b] = 0u;
+                if (rc) for (int b = 0; b <= kRecheckBuckets; b++) a.recheck_count[b] = 0u;
                 __threadfence();
             }
         }
