@@ -302,7 +302,7 @@ def make_roofline(info, w, m, world=1, key=None):
              "dtype": "3xTF32 (fp32 accumulate)",
              "tensor_tflops_executed": achieved * 3.0 * (info["d_pad"] + 8.0) / (w.d + w.m),     # K padded to d_pad + one 8-wide input block
              "fp32_alu_frac_whole_tick": work / (total_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
-             "second_pass": {"kernel": "rollout_reg_kernel (FP32, deferred candidates)" if info["d_pad"] <= 32 else "rollout_tile_kernel (FP32, deferred candidates)",
+             "second_pass": {"kernel": "rollout_split_kernel / rollout_reg_kernel (FP32, deferred candidates)" if info["d_pad"] <= 32 else "rollout_tile_kernel (FP32, deferred candidates)",
                              "ms_per_tick": second_ms / K_, "share_of_tick": second_ms / total_ms,
                              "deferred_fraction": info.get("deferred_fraction")}}
     else:
@@ -486,7 +486,7 @@ def main():
                     help="BASELINE.json configs[3] alone: N = 2^14 .. 2^20 on the C4 model, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
                     help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
-    ap.add_argument("--tensor32", action="store_true", help="d = 32: take the verified tensor-core tick below 2^17 candidates too (it is the default from 2^17)")
+    ap.add_argument("--tensor32", action="store_true", help="d = 32: take the verified tensor-core tick below 2^16 candidates too (it is the default from 2^16)")
     ap.add_argument("--unverified", action="store_true", help="tensor-core kernels without the verification pass (measurement only: the bare 3xTF32 rollout)")
     ap.add_argument("--no-predict", action="store_true", help="d > 32: pre-sort by input-box cell instead of by predicted life time")
     ap.add_argument("--no-tensor", action="store_true", help="FP32 kernels only (d = 32: register kernel, d = 128: SIMT warp-tile kernel)")

@@ -25,6 +25,7 @@ UNITS += [(f"lat{d}", "inst_lat.cu", [f"-DMPMI_D={d}"]) for d in (32, 16, 8)]
 UNITS += [(f"regn{d}_{m}", "inst_reg.cu", [f"-DMPMI_D={d}", f"-DMPMI_MODE={m}", "-DMPMI_NOISE=1"]) for d in (32, 16, 8) for m in (0, 1)]
 UNITS += [(f"tilen{d}_{m}", "inst_tile.cu", [f"-DMPMI_D={d}", f"-DMPMI_MODE={m}", "-DMPMI_NOISE=1"]) for d in (128, 64) for m in (0, 1)]
 UNITS += [("relift", "inst_relift.cu", []), ("affine", "inst_affine.cu", [])]
+UNITS += [("split", "inst_split.cu", []), ("splitn", "inst_split.cu", ["-DMPMI_NOISE=1"])]
 UNITS += [(f"tc_{m}", "inst_tc.cu", [f"-DMPMI_MODE={m}"]) for m in (0, 1)]
 UNITS += [(f"tile{d}_{m}", "inst_tile.cu", [f"-DMPMI_D={d}", f"-DMPMI_MODE={m}"]) for d in (128, 64) for m in (0, 1)]
 

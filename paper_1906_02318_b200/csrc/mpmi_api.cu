@@ -23,6 +23,7 @@
 #include "kernel_args.cuh"
 #include "binning.cuh"
 #include "bound.cuh"
+#include "rollout_split.cuh"
 
 using namespace mpmi;
 
@@ -118,7 +119,7 @@ namespace {
 
 constexpr unsigned kProfRing = 64;
 constexpr long long kLatMaxCand = 24576;        // <= this many candidates: latency kernel (measured: 125 vs 155 us at 2^14, 210 vs 164 us at 2^15)
-constexpr long long kTc32MinCand = 1LL << 17;   // D = 32: tensor-core kernel from this many candidates (four CTAs per SM need >= 592 tiles to fill)
+constexpr long long kTc32MinCand = 1LL << 16;   // D = 32: tensor-core kernel from this many candidates (four CTAs per SM need >= 592 tiles to fill)
 
 thread_local std::string g_create_err;
 
@@ -157,6 +158,7 @@ MPMI_DECL_REG(8) MPMI_DECL_REG(16) MPMI_DECL_REG(32) MPMI_DECL_TILE(64) MPMI_DEC
 KernFn mpmi_pick_tile_128_tick_rc(int M, int *smem); KernFn mpmi_pick_tile_128_batch_rc(int M, int *smem);
 KernFn mpmi_pick_tilen_128_tick_rc(int M, int *smem); KernFn mpmi_pick_tilen_128_batch_rc(int M, int *smem);
 KernFn mpmi_pick_reg_32_recheck(int M, int kconst); KernFn mpmi_pick_regn_32_recheck(int M, int kconst);
+KernFn mpmi_pick_split_32(int M, int rs); KernFn mpmi_pick_splitn_32(int M, int rs);
 KernFn mpmi_pick_relift(int n, int mode);
 KernFn mpmi_pick_affine_base(int D); KernFn mpmi_pick_affine(int np, int mode);
 KernFn mpmi_pick_tc_tick(int D, int *smem, int *threads, int *ctas_per_sm, int noise); KernFn mpmi_pick_tc_batch(int D, int *smem, int *threads, int *ctas_per_sm, int noise);
@@ -616,11 +618,26 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     CUC(cudaHostGetDevicePointer((void **)&c->d_res_mapped, c->h_res, 0));
     c->d_deferred_mapped = &reinterpret_cast<HostBlock *>(c->d_res_mapped)->deferred;
 
+    // ---- kernel choice ------------------------------------------------------------------------------
+    // prediction noise (Alg. 2 l.5) is built into the register, warp-tile, tensor-core (n <= 8) and re-lift kernels;
+    // the latency kernel does not carry it, so sigma != 0 routes around it
+    const bool noise = cfg->noise_sigma != 0.f;
+    dc.noise_sigma = cfg->noise_sigma; dc.model = cfg->model;
+    const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16;
+    const size_t aff_smem = (size_t)cfg->H * (1 + m) * NPn * sizeof(float);
+    // tensor cores: linear lifted model only; noise block holds 8 dims; the verification tables (bound.cuh) must fit
+    const bool tc_unverified = (cfg->variant & MPMI_VARIANT_TC_UNVERIFIED) != 0;
+    const bool tc_model_ok = cfg->model == MPMI_MODEL_LINEAR && (!noise || n <= 8) &&
+                             !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_AFFINE)) &&
+                             (tc_unverified || ((size_t)cfg->H * D * D * sizeof(float) <= ((size_t)256 << 20) && aff_smem <= 200 * 1024));
     // ---- spatial binning: large Philox candidate sets only (the grid is already spatially ordered)
     {
         const long long send = sb + sc < cfg->N ? sb + sc : cfg->N;
         const long long nsamp = send > sb ? send - sb : 0;
-        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (D > 32 ? (1 << 15) : (1 << 17));   // measured at d = 32: the ~25 us of binning pay from 2^17 up
+        // measured at d = 32: the ~25 us of binning pay from 2^17 candidates for the register kernel (a warp of 64 candidates), from
+        // 2^16 for the tensor-core tick (a tile of 128 candidates runs until its last one stops)
+        const bool tc32 = D == 32 && tc_model_ok && cfg->model == MPMI_MODEL_LINEAR;
+        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (D > 32 ? (1 << 15) : tc32 ? (1 << 16) : (1 << 17));
         c->binning = (cfg->variant & MPMI_VARIANT_FORCE_BINNING) ? (cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= 64)
                                                                   : (want && !(cfg->variant & MPMI_VARIANT_NO_BINNING));
         if (c->binning) {
@@ -640,18 +657,6 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         }
     }
 
-    // ---- kernel choice ------------------------------------------------------------------------------
-    // prediction noise (Alg. 2 l.5) is built into the register, warp-tile, tensor-core (n <= 8) and re-lift kernels;
-    // the latency kernel does not carry it, so sigma != 0 routes around it
-    const bool noise = cfg->noise_sigma != 0.f;
-    dc.noise_sigma = cfg->noise_sigma; dc.model = cfg->model;
-    const int NPn = n <= 4 ? 4 : n <= 8 ? 8 : 16;
-    const size_t aff_smem = (size_t)cfg->H * (1 + m) * NPn * sizeof(float);
-    // tensor cores: linear lifted model only; noise block holds 8 dims; the verification tables (bound.cuh) must fit
-    const bool tc_unverified = (cfg->variant & MPMI_VARIANT_TC_UNVERIFIED) != 0;
-    const bool tc_model_ok = cfg->model == MPMI_MODEL_LINEAR && (!noise || n <= 8) &&
-                             !(cfg->variant & (MPMI_VARIANT_NO_TENSOR | MPMI_VARIANT_AFFINE)) &&
-                             (tc_unverified || ((size_t)cfg->H * D * D * sizeof(float) <= ((size_t)256 << 20) && aff_smem <= 200 * 1024));
     bool tensor = false, tc32_batch = false;
     if (cfg->model == MPMI_MODEL_RELIFT) {
         // x' = C (K Psi(x) + B u): one thread per candidate, only the physical rows of the model (rollout_relift.cuh)
@@ -818,12 +823,25 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         if (D == 32) {               // FP32 register kernel, 2 candidates per thread, CTAs loop over blocks of the lists
             const int rc_kconst = (c->kslot >= 0 && !std::getenv("MPMI_RC_SMEM")) ? 1 : 0;
             c->k_recheck = noise ? mpmi_pick_regn_32_recheck(M, rc_kconst) : mpmi_pick_reg_32_recheck(M, rc_kconst);
+            // lanes per candidate pair in the second pass (measured, rollout_split.cuh): 4 up to 2^19 candidates, 2 beyond
+            // (0: one thread per pair, rollout_reg_kernel -- when the shared-memory model is forced, or MPMI_RC_RS=0)
+            int rc_rs = sc <= (1LL << 19) ? 4 : 2;
+            if (const char *e = std::getenv("MPMI_RC_RS")) rc_rs = std::atoi(e);
+            if (rc_rs == 2 || rc_rs == 4) {
+                // row-split kernel, one-warp CTAs rolling blocks of 64 / RS candidates, 16 per SM: the pass is set by how long ONE
+                // warp needs for the horizon, and RS lanes per pair cut that RS-fold (measured on C4, 3.8 % of 2^20 candidates:
+                // one thread per pair 250 us however the blocks are dealt out)
+                c->k_recheck = noise ? mpmi_pick_splitn_32(M, rc_rs) : mpmi_pick_split_32(M, rc_rs);
+                c->recheck_block = 32; c->recheck_smem = 0; c->recheck_persistent = false;
+                const long long per = 64 / rc_rs, nb = (sc + per - 1) / per, cap = 16LL * c->sm_count;
+                c->recheck_grid = (unsigned)(nb < cap ? nb : cap);
+            } else {
             // 4 one-warp CTAs per SM (one per sub-partition), each rolling blocks of 64 candidates: its own first, then first come,
-            // first served (rollout_reg.cuh).  Measured on C4 (3.8 % of 2^20 candidates deferred): 4-warp CTAs of 256 candidates
-            // with a static walk 260 us -- the SMs that got two of the long-lived head blocks set the time.
+            // first served (rollout_reg.cuh).
             c->recheck_block = 32; c->recheck_smem = 0; c->recheck_persistent = false;
             const long long nb = (sc + 63) / 64, cap = 4LL * c->sm_count;
             c->recheck_grid = (unsigned)(nb < cap ? nb : cap);
+            }
         } else {                     // FP32 warp-tile kernel, persistent CTAs fetch batches of the lists from the work counter
             int bs = 0;
             c->k_recheck = noise ? mpmi_pick_tilen_128_tick_rc(M, &c->recheck_smem) : mpmi_pick_tile_128_tick_rc(M, &c->recheck_smem);
