@@ -460,6 +460,60 @@ def run_sweep(args, local):
                       "sweep": s["rows"], "clocks": s["clocks"]}))
 
 
+def run_timeline(args, local):
+    """Where a paper-scale tick spends its time: %globaltimer stamps of the latency kernel's stages
+    (mpmi_profile_timeline) on device-resident ticks, and the host's view of mpmi_step / mpmi_step_result."""
+    import torch
+    import workloads as W
+    import paper_1906_02318_b200 as mp
+    stream = torch.cuda.current_stream().cuda_stream
+    w = W.make(args.workload)
+    ctx = mp.Context(w, device=local)
+    info = ctx.info()
+    nt = 300
+    x0s, uus, ticks = W.tick_inputs(w, nt)
+    dX0 = torch.as_tensor(x0s).cuda().contiguous(); dUU = torch.as_tensor(uus).cuda().contiguous()
+    dRes = torch.zeros(56, dtype=torch.uint8, device="cuda")
+    stamps = torch.zeros((info["blocks"], 8), dtype=torch.int64, device="cuda")
+    ctx.profile_timeline(stamps.data_ptr())
+    rows, ev_us = [], []
+    with clocked(local) as ck:
+        for t in range(nt):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.step_device(dX0[t].data_ptr(), dUU[t].data_ptr(), int(ticks[t]), stream, dRes.data_ptr())
+            e1.record()
+            torch.cuda.synchronize()
+            s = stamps.cpu().numpy().astype(np.int64)
+            if t >= 50:
+                t0 = s[:, 0].min()
+                rows.append([s[:, 0].max() - t0, np.median(s[:, 1] - s[:, 0]), np.median(s[:, 2] - s[:, 1]), np.median(s[:, 3] - s[:, 2]),
+                             np.median(s[:, 4] - s[:, 3]), (s[:, 4] - s[:, 3]).max(), np.median(s[:, 5] - s[:, 4]), s[:, 5].max() - t0,
+                             s[:, 4].max() - t0])
+                ev_us.append(1e3 * e0.elapsed_time(e1))
+        ctx.profile_timeline(0)
+        r = np.median(np.array(rows, dtype=np.float64), axis=0) / 1e3
+        # host view
+        xs = [np.ascontiguousarray(x) for x in x0s]; us = [np.ascontiguousarray(u) for u in uus]
+        t_enq, t_wait, t_tot = [], [], []
+        for t in range(nt):
+            a0 = time.perf_counter(); ctx.step(xs[t], us[t], int(ticks[t]), stream)
+            a1 = time.perf_counter(); ctx.step_result()
+            a2 = time.perf_counter()
+            if t >= 50:
+                t_enq.append(a1 - a0); t_wait.append(a2 - a1); t_tot.append(a2 - a0)
+    med = lambda v: 1e6 * float(np.median(v))
+    print(json.dumps({
+        "metric": "tick timeline", "workload": f"{args.workload}: n={w.n} m={w.m} d={w.d} N={w.N} H={w.H}", "kernel": info, "ticks": nt - 50,
+        "device_us_median": {"first CTA start -> last CTA start": r[0], "entry -> model rows requested": r[1], "-> lift done + __syncthreads": r[2],
+                             "-> candidate sampled, state initialised": r[3], "-> horizon loop left (median CTA)": r[4], "horizon loop (slowest CTA)": r[5],
+                             "-> keys reduced, ticket taken": r[6], "first CTA start -> last CTA leaves the horizon loop": r[8],
+                             "first CTA start -> last CTA done (kernel span)": r[7], "CUDA events around the launch": float(np.median(ev_us))},
+        "host_us_median": {"mpmi_step (copy inputs, 1 node-param update, cudaGraphLaunch)": med(t_enq),
+                           "mpmi_step_result (poll the mapped result)": med(t_wait), "total": med(t_tot)},
+        "clocks": ck.summary}))
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
@@ -482,6 +536,7 @@ def main():
     ap.add_argument("--noise", type=float, default=0.0,
                     help="std of the additive prediction noise of Alg. 2 l.5 (PAPER.md:150); 0 = the noise-free configs of BASELINE.json")
     ap.add_argument("--relift", action="store_true", help="re-lift model x' = C(K Psi(x) + B u) instead of the linear lifted model")
+    ap.add_argument("--timeline", action="store_true", help="stage timeline of a paper-scale tick (latency kernel: C1, C2, C3) instead of the bench line")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[3] alone: N = 2^14 .. 2^20 on the C4 model, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
@@ -531,6 +586,8 @@ def main():
     stream = torch.cuda.current_stream().cuda_stream
     if args.sweep:
         return run_sweep(args, local)
+    if args.timeline:
+        return run_timeline(args, local)
 
     # ---- workload: weak scaling -- every rank owns N_per candidates of a global set of world*N_per
     w1 = W.make(args.workload, N=args.N)

@@ -213,6 +213,11 @@ int mpmi_step_trace(mpmi_ctx *ctx, const float *d_x0, const float *d_u_user, uin
  * recorded ticks and returns, oldest first, the device time of the tick kernel and of the second pass (0 if there is
  * none) of the last `*count` <= min(capacity, 64) ticks, in milliseconds (host arrays). */
 int mpmi_profile_enable(mpmi_ctx *ctx, int32_t enable);
+/* Stage timeline of a paper-scale tick (latency kernel, info.variant == 3; else UNSUPPORTED): while d_stamps (device,
+ * 8 * info.blocks uint64) is set, the plain-launch entries make thread 0 of every CTA store %globaltimer (ns) at
+ * [0] kernel entry, [1] model rows requested, [2] lift done, [3] candidate sampled, [4] horizon loop left,
+ * [5] keys reduced and ticket taken; NULL switches it off. */
+int mpmi_profile_timeline(mpmi_ctx *ctx, uint64_t *d_stamps);
 int mpmi_profile_read(mpmi_ctx *ctx, int32_t capacity, int32_t *count, float *ms_tick_kernel, float *ms_second_pass);
 
 /* Sharded tick (section 8(e)): roll out this context's shard and write its mpmi_partial to

@@ -32,6 +32,7 @@ struct KArgs {
     int recheck_mode;                     // register kernel: 1 = walk the recheck lists (longest-lived first) instead of the index space
     float recheck_tau_scale;              // scales tau (1 = the derived bound; MPMI_TC_TAU_SCALE < 1 measures how conservative it is)
     int *deferred_out;                    // host-mapped: candidates the second pass rolled (mpmi_info.reserved), or null
+    unsigned long long *timeline;         // device, 8 x gridDim %globaltimer stamps of the latency kernel's stages (mpmi_profile_timeline), or null
     // batch
     const float *U;                       // device Ncand*m or null
     long long x0_count;

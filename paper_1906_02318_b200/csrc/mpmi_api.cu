@@ -92,6 +92,7 @@ struct mpmi_ctx {
     int *d_deferred_mapped = nullptr;
     KArgs gr{};
     // mpmi_profile_enable: CUDA events around the tick kernel and the second pass of the plain-launch entries (ring of kProfRing ticks)
+    unsigned long long *timeline = nullptr;   // mpmi_profile_timeline: caller's device buffer, or null
     bool prof = false;
     std::vector<cudaEvent_t> prof_ev;     // 3 per slot: before the tick kernel, after it, after the second pass
     unsigned prof_n = 0;
@@ -315,6 +316,7 @@ cudaError_t enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         a.recheck = c->d_recheck; a.recheck_count = c->d_recheck_count; a.recheck_mode = 0; a.recheck_tau_scale = c->recheck_tau_scale;
         if (fork) CL(cudaStreamWaitEvent(s, c->ev_join, 0));
     }
+    a.timeline = c->timeline;
     cudaEvent_t *pe = c->prof ? const_cast<cudaEvent_t *>(&c->prof_ev[3 * (c->prof_n % kProfRing)]) : nullptr;
     if (pe) CL(cudaEventRecord(pe[0], s));
     CL(launch(c, c->k_tick, c->dc.shard_count, a, s));
@@ -990,6 +992,8 @@ int mpmi_step(mpmi_ctx *c, const float *x0, const float *u_user, uint64_t tick, 
     c->ga.tick_val = tick;
     if (++c->seq == 0) c->seq = 1;
     c->ga.seq = c->seq;
+    // (a one-kernel tick goes through its one-node graph as well: measured on C1 / C2 / C3, cudaLaunchKernel with the ~1.2 KB of
+    // by-value kernel parameters costs 10.3 us of host time per tick, node-parameter update + cudaGraphLaunch 6.5 us)
     cudaKernelNodeParams p; void *args[2];
     if (c->binning) {
         c->gb.tick_val = tick;
@@ -1080,6 +1084,13 @@ int mpmi_profile_enable(mpmi_ctx *c, int32_t enable) {
         for (cudaEvent_t &e : c->prof_ev) CU(c, cudaEventCreate(&e));
     }
     c->prof = enable != 0; c->prof_n = 0;
+    return MPMI_OK;
+}
+
+int mpmi_profile_timeline(mpmi_ctx *c, uint64_t *d_stamps) {
+    if (!c) return MPMI_ERR_INVALID;
+    if (d_stamps && c->variant != 3) return fail(c, MPMI_ERR_UNSUPPORTED, "the stage timeline is recorded by the latency kernel (paper-scale candidate sets)");
+    c->timeline = reinterpret_cast<unsigned long long *>(d_stamps);
     return MPMI_OK;
 }
 

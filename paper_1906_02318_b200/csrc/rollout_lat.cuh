@@ -25,6 +25,10 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     __shared__ float sz0[D];
 
     const int tid = threadIdx.x, lane = tid & 31, q = lane & (L - 1);
+    // mpmi_profile_timeline: thread 0 of every CTA stamps the stages (ns, %globaltimer); a.timeline == null costs one uniform branch each
+    unsigned long long *tl = a.timeline ? a.timeline + 8ull * blockIdx.x : nullptr;
+#define MPMI_STAMP(i) do { if (tl && tid == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); tl[i] = t_; } } while (0)
+    MPMI_STAMP(0);                                // kernel entry
     // this lane's rows of the augmented transposed model, as row pairs
     float2 kreg[D + M][R / 2];
     {
@@ -34,6 +38,7 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
             for (int p = 0; p < R / 2; p++) kreg[c][p] = __ldg(kt + (c * D) / 2 + p);
     }
+    MPMI_STAMP(1);                                // model rows requested (the loads are still in flight)
     const unsigned long long tick = a.tick_val;
     const float *x0p = a.inline_inputs ? a.x0_val : a.x0;
     const float *uup = a.inline_inputs ? a.u_val : a.u_user;
@@ -45,6 +50,7 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     clamp_user(cfg, uup, u_h);
     for (int f = tid; f < D; f += kLatBlock) sz0[f] = lift_feature(cfg, f, x0p);
     __syncthreads();
+    MPMI_STAMP(2);                                // lift done, CTA synchronised
 
     // ---- a1 + a2 ----------------------------------------------------------------------------------
     const long long li = (long long)blockIdx.x * (kLatBlock / L) + tid / L;
@@ -59,13 +65,15 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
         for (int c = 0; c < D; c++) z[c] = sz0[c];
     }
+    MPMI_STAMP(3);                                // candidate sampled (Philox / grid), state initialised
     const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
     const bool no_annulus = cfg.annulus == 0;
     // only constrained dims are tested (as in every other kernel and in the oracle): an unconstrained dim passes whatever
-    // it holds, Inf and NaN included -- its (-inf, +inf) limits alone would reject those
-    bool unc[NB];
+    // it holds, Inf and NaN included -- its (-inf, +inf) limits alone would reject those.  One AND per dim: the state's bit
+    // pattern is masked to +0.0 where the dim is unconstrained, and 0 lies inside (-inf, +inf).
+    unsigned zm[NB];
 #pragma unroll
-    for (int j = 0; j < NB; j++) unc[j] = ((cfg.bmask >> j) & 1u) == 0u;
+    for (int j = 0; j < NB; j++) zm[j] = ((cfg.bmask >> j) & 1u) ? 0xFFFFFFFFu : 0u;
 
     // ---- a3 + a4: no memory traffic inside this loop -----------------------------------------------
     for (int k = 0; k < H; k++) {
@@ -93,7 +101,10 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         // none), the annulus folded in arithmetically; only more than 4 boxed dims take a branch
         bool ok = true;
 #pragma unroll
-        for (int j = 0; j < 4 && j < NB; j++) ok = ok & (((z[j] > cfg.blo[j]) & (z[j] < cfg.bhi[j])) | unc[j]);
+        for (int j = 0; j < 4 && j < NB; j++) {
+            const float zt = __uint_as_float(__float_as_uint(z[j]) & zm[j]);
+            ok = ok & (zt > cfg.blo[j]) & (zt < cfg.bhi[j]);
+        }
         {
             const float dx = __fsub_rn(z[0], cfg.cx), dy = __fsub_rn(z[1], cfg.cy);
             const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
@@ -101,12 +112,16 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         }
         if (nbox > 4) {
 #pragma unroll
-            for (int j = 4; j < NB; j++) ok = ok & (((z[j] > cfg.blo[j]) & (z[j] < cfg.bhi[j])) | unc[j]);
+            for (int j = 4; j < NB; j++) {
+                const float zt = __uint_as_float(__float_as_uint(z[j]) & zm[j]);
+                ok = ok & (zt > cfg.blo[j]) & (zt < cfg.bhi[j]);
+            }
         }
         alive = alive & ok;
         steps += alive ? 1 : 0;
     }
 
+    MPMI_STAMP(4);                                // horizon loop left (warp 0 of the CTA)
     // ---- a5-a7 ------------------------------------------------------------------------------------
     unsigned long long key = kKeyNone;
     unsigned n_safe = 0, n_exec = 0;
@@ -124,6 +139,8 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         n_exec = (unsigned)(steps + 1 < H ? steps + 1 : H);
     }
     block_select_and_finalise<kLatBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq);
+    MPMI_STAMP(5);                                // keys reduced, ticket taken (last CTA: result written)
+#undef MPMI_STAMP
 }
 
 }  // namespace mpmi

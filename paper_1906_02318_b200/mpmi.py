@@ -19,7 +19,7 @@ VARIANT_LAT_R2, VARIANT_LAT_R4, VARIANT_NO_TENSOR, VARIANT_AFFINE, VARIANT_NO_PR
 VARIANT_TENSOR32, VARIANT_SMEM_MODEL, VARIANT_TC_UNVERIFIED = 1024, 2048, 4096
 
 EXPORTS = ("mpmi_create", "mpmi_destroy", "mpmi_step", "mpmi_step_result", "mpmi_step_sync",
-           "mpmi_step_device", "mpmi_step_trace", "mpmi_profile_enable", "mpmi_profile_read", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
+           "mpmi_step_device", "mpmi_step_trace", "mpmi_profile_enable", "mpmi_profile_timeline", "mpmi_profile_read", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
            "mpmi_get_info", "mpmi_strerror", "mpmi_last_error")
 
 
@@ -101,6 +101,7 @@ def load_library():
     lib.mpmi_step_device.argtypes = [vp, vp, vp, u64, vp, vp]
     lib.mpmi_step_trace.argtypes = [vp, vp, vp, u64, vp, vp, vp]
     lib.mpmi_profile_enable.argtypes = [vp, i32]
+    lib.mpmi_profile_timeline.argtypes = [vp, vp]
     lib.mpmi_profile_read.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.mpmi_shard_step.argtypes = [vp, vp, vp, u64, vp, vp]
     lib.mpmi_shard_finalize.argtypes = [vp, vp, i32, vp, u64, vp, vp]
@@ -215,6 +216,9 @@ class Context:
 
     def profile_enable(self, enable=True):
         self._check(self._lib.mpmi_profile_enable(self._h, 1 if enable else 0))
+
+    def profile_timeline(self, d_stamps):
+        self._check(self._lib.mpmi_profile_timeline(self._h, d_stamps))
 
     def profile_read(self, capacity=64):
         """(ms of the tick kernel, ms of the second pass) per recorded plain-launch tick, oldest first"""
