@@ -254,82 +254,79 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
     unsigned n_safe = 0, n_exec = 0;
 
     if (warp == kTcStateWarps) {
-        // ================= MMA issuer: one elected lane ==============================================
-        if (lane == 0) {
+        // ================= MMA issuer ====================================================================
+        // The whole warp runs this loop CONVERGENTLY and one elected lane issues the MMAs (elect.sync): every tcgen05.mma
+        // operand (TMEM addresses, shared-memory descriptors) is then a warp-uniform value that ptxas can keep in uniform
+        // registers.  With the loop inside `if (lane == 0)` (round 1) every operand lived in a vector register of a divergent
+        // region and each MMA was wrapped in an ELECT / R2UR.BROADCAST sequence, ~49 clk per MMA.
+        {
+            const uint32_t tbu = __reduce_max_sync(0xffffffffu, tb);          // uniform by construction
             const uint32_t idesc = idesc_tf32(kTcTile, kTcD);
             const uint64_t dhi = smem_desc_kmajor(smem_u32(smem_img), kTcLBO, kTcSBO);
             const uint64_t dlo = smem_desc_kmajor(smem_u32(smem_img + kTcImg), kTcLBO, kTcSBO);
             constexpr uint64_t kstep = (2 * kTcLBO) >> 4;                 // descriptor address units per k-block
-            unsigned p_full = 0, p_alo = 0, it = 0;
-#ifdef MPMI_TC_DEBUG
-            long long tw_full = 0, ti_1 = 0, tw_alo = 0, ti_23 = 0, nsteps = 0, tq = 0;
-#define TCT(acc) do { long long t_ = clock64(); acc += t_ - tq; tq = t_; } while (0)
-#else
-#define TCT(acc) do {} while (0)
-#endif
-            for (;; it++) {
-                const unsigned tile = atomicAdd(a.work, 1u);
-                sh.tile[it & 1] = tile;
-                mbar_arrive(bar_tile);
+            unsigned p_full = 0, p_alo = 0;
+            auto tile_alive = [&]() { return (sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3]) != 0u; };
+            for (unsigned it = 0;; it++) {
+                unsigned tile = 0;
+                if (lane == 0) tile = atomicAdd(a.work, 1u);
+                tile = __shfl_sync(0xffffffffu, tile, 0);
+                if (lane == 0) { sh.tile[it & 1] = tile; mbar_arrive(bar_tile); }
+                __syncwarp();
                 if (tile >= ntile) break;
                 for (int s = 0; s < H; s++) {
-                    const uint32_t dcur = tb + ((s & 1) ? kTcColD1 : kTcColD0), dnxt = tb + ((s & 1) ? kTcColD0 : kTcColD1);
-#ifdef MPMI_TC_DEBUG
-                    tq = clock64(); nsteps++;
-#endif
+                    const uint32_t dcur = tbu + ((s & 1) ? kTcColD1 : kTcColD0), dnxt = tbu + ((s & 1) ? kTcColD0 : kTcColD1);
                     // z_s complete in TMEM: written by the previous step's MMAs (s > 0) or by the prologue (s = 0)
                     if (s > 0) { mbar_wait(bar_full, p_full); p_full ^= 1; }
                     else { mbar_wait(bar_alo, p_alo); p_alo ^= 1; }
                     fence_after_sync();
-                    TCT(tw_full);
-#ifdef MPMI_TC_DEBUG
-                    if (s > 0) *reinterpret_cast<volatile long long *>(&sh.dbg_wake) = clock64();
-#endif
                     // The small products go first: the tensor core accumulates with truncation toward zero
                     // (measured), so terms added while the accumulator is still ~2^-11 |z| lose nothing that
-                    // matters, and only the 17 accumulations of Z_hi * K_hi run at full magnitude.
-                    if (s == 0 && !(sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3])) {
-                        sh.stop_tile = tile; mbar_arrive(bar_full); break;                  // nothing valid in this tile
+                    // matters, and only the accumulations of Z_hi * K_hi run at full magnitude.
+                    if (s == 0 && !tile_alive()) {                         // nothing valid in this tile
+                        if (lane == 0) { sh.stop_tile = tile; mbar_arrive(bar_full); }
+                        __syncwarp();
+                        break;
                     }
                     constexpr int kSplit = G::kSplit;                      // k-blocks of group 1 issued before the hand-back wait
+                    if (elect_one()) {
 #pragma unroll
-                    for (int kk = 0; kk < kSplit; kk++)                    // Z_hi * K_lo  (Z_hi = the fp32 state itself)
-                        mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tb + kTcColU, dlo + kk * kstep, idesc, kk > 0);
-                    TCT(ti_1);
+                        for (int kk = 0; kk < kSplit; kk++)                // Z_hi * K_lo  (Z_hi = the fp32 state itself)
+                            mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tbu + kTcColU, dlo + kk * kstep, idesc, kk > 0);
+                    }
+                    __syncwarp();
                     if (s > 0) {                                           // state warps: z_s tested, Z_lo written
                         mbar_wait(bar_alo, p_alo); p_alo ^= 1;             // (its latency hides behind the queued MMAs)
                         fence_after_sync();
-                        if (!(sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3])) {
-                            sh.stop_tile = tile; mma_commit(bar_full); break;               // stop: drains, then wakes them
+                        if (!tile_alive()) {                               // stop: the queued MMAs drain, then the commit wakes the state warps
+                            if (elect_one()) { sh.stop_tile = tile; mma_commit(bar_full); }
+                            __syncwarp();
+                            break;
                         }
                     }
-                    TCT(tw_alo);
+                    if (elect_one()) {
 #pragma unroll
-                    for (int kk = kSplit; kk < kTcKB + 1; kk++)            // (last k-block: u_hi * B_lo)
-                        mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tb + kTcColU, dlo + kk * kstep, idesc, true);
+                        for (int kk = kSplit; kk < kTcKB + 1; kk++)        // (last k-block: u_hi * B_lo)
+                            mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tbu + kTcColU, dlo + kk * kstep, idesc, true);
 #pragma unroll
-                    for (int kk = 0; kk < kTcKB; kk++)                     // Z_lo * K_hi
-                        mma_tf32_ts(dnxt, tb + kTcColAlo + 8 * kk, dhi + kk * kstep, idesc, true);
-                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNlo, dhi + (kTcKB + 1) * kstep, idesc, true);     // (sigma eps)_lo through the selector
-                    // Z_hi * K_hi, the only products at full magnitude, in DESCENDING k-block order: input block ((u_hi + u_lo) * B_hi),
-                    // (sigma eps)_hi, then the state blocks KB-1 .. 0.  Every accumulation truncates the running sum (<= 2 ulp), so the
-                    // block of the physical dims (columns 0..7), the dominant one of a physical row when K is close to the identity
-                    // there, goes last and is truncated once (csrc/bound.cuh weighs block b with b + 1 accumulations).
-                    mma_tf32_ts(dnxt, tb + kTcColU, dhi + kTcKB * kstep, idesc, true);
-                    if (NOISE) mma_tf32_ts(dnxt, tb + kTcColNhi, dhi + (kTcKB + 1) * kstep, idesc, true);
+                        for (int kk = 0; kk < kTcKB; kk++)                 // Z_lo * K_hi
+                            mma_tf32_ts(dnxt, tbu + kTcColAlo + 8 * kk, dhi + kk * kstep, idesc, true);
+                        if (NOISE) mma_tf32_ts(dnxt, tbu + kTcColNlo, dhi + (kTcKB + 1) * kstep, idesc, true);     // (sigma eps)_lo through the selector
+                        // Z_hi * K_hi, the only products at full magnitude, in DESCENDING k-block order: input block ((u_hi + u_lo) * B_hi),
+                        // (sigma eps)_hi, then the state blocks KB-1 .. 0.  Every accumulation truncates the running sum (<= 2 ulp), so the
+                        // block of the physical dims (columns 0..7), the dominant one of a physical row when K is close to the identity
+                        // there, goes last and is truncated once (csrc/bound.cuh weighs block b with b + 1 accumulations).
+                        mma_tf32_ts(dnxt, tbu + kTcColU, dhi + kTcKB * kstep, idesc, true);
+                        if (NOISE) mma_tf32_ts(dnxt, tbu + kTcColNhi, dhi + (kTcKB + 1) * kstep, idesc, true);
 #pragma unroll
-                    for (int kk = kTcKB - 1; kk >= 0; kk--)
-                        mma_tf32_ts(dnxt, dcur + 8 * kk, dhi + kk * kstep, idesc, true);
-                    mma_commit(bar_full);
-                    TCT(ti_23);
+                        for (int kk = kTcKB - 1; kk >= 0; kk--)
+                            mma_tf32_ts(dnxt, dcur + 8 * kk, dhi + kk * kstep, idesc, true);
+                        mma_commit(bar_full);
+                    }
+                    __syncwarp();
                 }
                 mbar_wait(bar_full, p_full); p_full ^= 1;                 // last commit (or the stop signal) of this tile
             }
-#ifdef MPMI_TC_DEBUG
-            if (blockIdx.x == 0 && nsteps > 0)
-                printf("tc timing (clk/step): wait_full %lld issue1 %lld wait_alo %lld issue23 %lld  steps %lld\n",
-                       tw_full / nsteps, ti_1 / nsteps, tw_alo / nsteps, ti_23 / nsteps, nsteps);
-#endif
         }
         __syncwarp();
     } else {
