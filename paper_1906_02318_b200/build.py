@@ -17,7 +17,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmpmi.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("MPMI_NVCC_EXTRA", "").split()     # e.g. -DMPMI_TC_DEBUG: in-kernel clock64 timelines
 
 UNITS = [("api", "mpmi_api.cu", [])]
 UNITS += [(f"reg{d}_{m}", "inst_reg.cu", [f"-DMPMI_D={d}", f"-DMPMI_MODE={m}"]) for d in (32, 16, 8) for m in (0, 1)]

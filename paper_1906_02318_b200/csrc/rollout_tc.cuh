@@ -42,6 +42,9 @@ constexpr int kTcLBO = 128;                       // bytes between 16-byte K chu
 #ifndef MPMI_TC_STATE_WARPS
 #define MPMI_TC_STATE_WARPS 8
 #endif
+#ifndef MPMI_TC32_STATE_WARPS
+#define MPMI_TC32_STATE_WARPS 4      // (8, i.e. 16 columns per thread at 56 registers, was measured slower: first pass 0.76 -> 0.82 ms)
+#endif
 // Geometry for padded lifted dim D = 128 (one CTA per SM, all 512 TMEM columns) and D = 32 (the same kernel with
 // N = 32 MMAs: a tile needs 3 D + 24 = 120 TMEM columns and 12 KB of operand images, so FOUR CTAs share an SM and
 // their step phases interleave -- measured: one CTA issues an M128 N32 K8 MMA every ~49 clk, four reach the 16 clk floor).
@@ -52,7 +55,7 @@ struct TcGeom {
     static constexpr int kKB = D / 8;                              // k-blocks of the state
     static constexpr int kKD = D + 16;                             // contraction length: D state + 8 input columns ([u_hi | u_lo], m <= 4)
                                                                    // + 8 noise columns (n <= 8; used by the NOISE instantiation only)
-    static constexpr int kStateWarps = D == 128 ? MPMI_TC_STATE_WARPS : 4;   // 4 lane quadrants x column groups
+    static constexpr int kStateWarps = D == 128 ? MPMI_TC_STATE_WARPS : MPMI_TC32_STATE_WARPS;   // 4 lane quadrants x column groups
     static constexpr int kCols = D / (kStateWarps / 4);            // state columns per state-warp thread
     static constexpr int kThreads = (kStateWarps + 1) * 32;
     static constexpr int kSBO = (kKD / 4) * 128;                   // bytes between 8-row groups
@@ -266,6 +269,12 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
             const uint64_t dlo = smem_desc_kmajor(smem_u32(smem_img + kTcImg), kTcLBO, kTcSBO);
             constexpr uint64_t kstep = (2 * kTcLBO) >> 4;                 // descriptor address units per k-block
             unsigned p_full = 0, p_alo = 0;
+#ifdef MPMI_TC_DEBUG
+            long long tw_full = 0, ti_1 = 0, tw_alo = 0, ti_23 = 0, nsteps = 0, tq = 0;
+#define TCT(acc) do { long long t_ = clock64(); acc += t_ - tq; tq = t_; } while (0)
+#else
+#define TCT(acc) do {} while (0)
+#endif
             auto tile_alive = [&]() { return (sh.warp_alive[0] | sh.warp_alive[1] | sh.warp_alive[2] | sh.warp_alive[3]) != 0u; };
             for (unsigned it = 0;; it++) {
                 unsigned tile = 0;
@@ -276,10 +285,17 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 if (tile >= ntile) break;
                 for (int s = 0; s < H; s++) {
                     const uint32_t dcur = tbu + ((s & 1) ? kTcColD1 : kTcColD0), dnxt = tbu + ((s & 1) ? kTcColD0 : kTcColD1);
+#ifdef MPMI_TC_DEBUG
+                    tq = clock64(); nsteps++;
+#endif
                     // z_s complete in TMEM: written by the previous step's MMAs (s > 0) or by the prologue (s = 0)
                     if (s > 0) { mbar_wait(bar_full, p_full); p_full ^= 1; }
                     else { mbar_wait(bar_alo, p_alo); p_alo ^= 1; }
                     fence_after_sync();
+                    TCT(tw_full);
+#ifdef MPMI_TC_DEBUG
+                    if (s > 0 && lane == 0) *reinterpret_cast<volatile long long *>(&sh.dbg_wake) = clock64();
+#endif
                     // The small products go first: the tensor core accumulates with truncation toward zero
                     // (measured), so terms added while the accumulator is still ~2^-11 |z| lose nothing that
                     // matters, and only the accumulations of Z_hi * K_hi run at full magnitude.
@@ -295,6 +311,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                             mma_tf32_ts(dnxt, kk < kTcKB ? dcur + 8 * kk : tbu + kTcColU, dlo + kk * kstep, idesc, kk > 0);
                     }
                     __syncwarp();
+                    TCT(ti_1);
                     if (s > 0) {                                           // state warps: z_s tested, Z_lo written
                         mbar_wait(bar_alo, p_alo); p_alo ^= 1;             // (its latency hides behind the queued MMAs)
                         fence_after_sync();
@@ -304,6 +321,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                             break;
                         }
                     }
+                    TCT(tw_alo);
                     if (elect_one()) {
 #pragma unroll
                         for (int kk = kSplit; kk < kTcKB + 1; kk++)        // (last k-block: u_hi * B_lo)
@@ -324,9 +342,15 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                         mma_commit(bar_full);
                     }
                     __syncwarp();
+                    TCT(ti_23);
                 }
                 mbar_wait(bar_full, p_full); p_full ^= 1;                 // last commit (or the stop signal) of this tile
             }
+#ifdef MPMI_TC_DEBUG
+            if (blockIdx.x == 0 && lane == 0 && nsteps > 0)
+                printf("tc timing (clk/step): wait_full %lld issue1 %lld wait_alo %lld issue23 %lld  steps %lld\n",
+                       tw_full / nsteps, ti_1 / nsteps, tw_alo / nsteps, ti_23 / nsteps, nsteps);
+#endif
         }
         __syncwarp();
     } else {

@@ -8,7 +8,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libmpmi.so")
+_LIB_PATH = os.environ.get("MPMI_LIB") or os.path.join(_HERE, "libmpmi.so")     # MPMI_LIB: e.g. a build with MPMI_NVCC_EXTRA=-DMPMI_TC_DEBUG
 
 SAMPLER_PHILOX, SAMPLER_GRID = 0, 1
 LIFT_MONO, LIFT_RFF = 0, 1
