@@ -37,8 +37,8 @@ namespace mpmi {
 constexpr int kTcTile = 128;                      // candidates per tile = TMEM lanes
 constexpr int kTcLBO = 128;                       // bytes between 16-byte K chunks (core matrices contiguous along K)
 #ifndef MPMI_TC_KSPLIT
-#define MPMI_TC_KSPLIT 15
-#endif
+#define MPMI_TC_KSPLIT 17            // d = 128: all 17 k-blocks of Z_hi * K_lo go out before the hand-back wait (measured with the
+#endif                               // convergent issue loop: 10 / 15 / 17 -> first pass 1.51 / 1.41 / 1.37 ms on C5)
 #ifndef MPMI_TC_STATE_WARPS
 #define MPMI_TC_STATE_WARPS 8
 #endif
