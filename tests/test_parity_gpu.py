@@ -826,3 +826,46 @@ def test_two_rank_nccl_sharded_tick(mp):
     out = tmp.Manager().dict()
     tmp.spawn(_nccl_worker, args=(2, 29500 + os.getpid() % 2000, name, N, nticks, out), nprocs=2, join=True)
     assert out[0] == ref and out[1] == ref
+
+
+# ------------------------------------------------------------------ measurement entry points ---------------------------
+def test_profile_entry_points(mp):
+    """mpmi_profile_enable / mpmi_profile_read: event times of the tick kernel and the second pass of plain-launch ticks;
+    mpmi_profile_timeline: stage stamps of the latency kernel (monotone per CTA), UNSUPPORTED on the other kernels.  The
+    tick's result is not affected by either."""
+    s = torch.cuda.current_stream().cuda_stream
+    w = W.make("C4", N=1 << 17)                               # verified tensor-core tick: both passes timed
+    ctx = mp.Context(w)
+    x0s, uus, ticks = W.tick_inputs(w, 5)
+    d_res = torch.zeros(56, dtype=torch.uint8, device="cuda")
+    ref = [ctx.step_sync(x0, uu, int(t)).as_dict(w.m) for x0, uu, t in zip(x0s, uus, ticks)]
+    ctx.profile_enable(True)
+    for k, (x0, uu, t) in enumerate(zip(x0s, uus, ticks)):
+        dx, du = _dev(x0), _dev(uu)
+        ctx.step_device(dx.data_ptr(), du.data_ptr(), int(t), s, d_res.data_ptr())
+        torch.cuda.synchronize()
+        got = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)[0]
+        assert int(got["key"]) == ref[k]["key"] and int(got["n_exec"]) == ref[k]["n_exec"]
+    first, second = ctx.profile_read()
+    ctx.profile_enable(False)
+    assert len(first) == 5 and len(second) == 5 and (first > 0.05).all() and (second > 0.005).all() and (first < 50).all()
+    with pytest.raises(mp.MpmiError) as e:
+        ctx.profile_timeline(d_res.data_ptr())
+    assert e.value.status == mp.mpmi.ERR_UNSUPPORTED
+    w2 = W.make("C2")                                         # latency kernel: the stage timeline
+    c2 = mp.Context(w2)
+    info = c2.info()
+    assert info["variant"] == 3
+    stamps = torch.zeros((info["blocks"], 8), dtype=torch.int64, device="cuda")
+    x0s, uus, ticks = W.tick_inputs(w2, 2)
+    want = c2.step_sync(x0s[1], uus[1], int(ticks[1])).as_dict(1)
+    c2.profile_timeline(stamps.data_ptr())
+    dx, du = _dev(x0s[1]), _dev(uus[1])
+    c2.step_device(dx.data_ptr(), du.data_ptr(), int(ticks[1]), s, d_res.data_ptr())
+    torch.cuda.synchronize()
+    c2.profile_timeline(0)
+    got = np.frombuffer(d_res.cpu().numpy().tobytes(), dtype=mp.mpmi.RESULT_DTYPE)[0]
+    assert int(got["key"]) == want["key"]
+    st = stamps.cpu().numpy()
+    assert (st[:, 0] > 0).all() and (np.diff(st[:, :6], axis=1) >= 0).all()
+    assert 1e3 < (st[:, 5].max() - st[:, 0].min()) < 1e6      # kernel span between 1 us and 1 ms
