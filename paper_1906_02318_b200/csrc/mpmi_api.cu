@@ -830,12 +830,14 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             int rc_rs = sc <= (1LL << 19) ? 4 : 2;
             if (const char *e = std::getenv("MPMI_RC_RS")) rc_rs = std::atoi(e);
             if (rc_rs == 2 || rc_rs == 4) {
-                // row-split kernel, one-warp CTAs rolling blocks of 64 / RS candidates, 16 per SM: the pass is set by how long ONE
+                // row-split kernel, one-warp CTAs rolling blocks of 64 / RS candidates, 8 per SM: the pass is set by how long ONE
                 // warp needs for the horizon, and RS lanes per pair cut that RS-fold (measured on C4, 3.8 % of 2^20 candidates:
                 // one thread per pair 250 us however the blocks are dealt out)
                 c->k_recheck = noise ? mpmi_pick_splitn_32(M, rc_rs) : mpmi_pick_split_32(M, rc_rs);
                 c->recheck_block = 32; c->recheck_smem = 0; c->recheck_persistent = false;
-                const long long per = 64 / rc_rs, nb = (sc + per - 1) / per, cap = 16LL * c->sm_count;
+                long long per_sm = 8;             // two persistent warps per sub-partition + first-come blocks (measured 4 / 6 / 8 / 10 / 16 per SM: 8 best at every N)
+                if (const char *e = std::getenv("MPMI_RC_CTAS")) per_sm = std::atoi(e) > 0 ? std::atoi(e) : per_sm;   // (measurement aid)
+                const long long per = 64 / rc_rs, nb = (sc + per - 1) / per, cap = per_sm * c->sm_count;
                 c->recheck_grid = (unsigned)(nb < cap ? nb : cap);
             } else {
             // 4 one-warp CTAs per SM (one per sub-partition), each rolling blocks of 64 candidates: its own first, then first come,

@@ -13,6 +13,8 @@
 // rollout_reg_kernel at every N: 2^16 candidates 322 / 542 us at RS = 2 / 4 against 271 us), so it serves the second pass only:
 // measured verified tick at 2^16 / 2^17 / 2^18 / 2^19 candidates 397 / 478 / 597 / 852 us with rollout_reg_kernel as second pass,
 // 241 / 321 / 452 / 760 us with RS = 4; at 2^20 (40,000 deferred: throughput-bound again) 1.32 ms against 1.30 ms with RS = 2.
+// (An all-gather through shared memory -- RL / 2 STS.128 + D / 2 LDS.128 per lane instead of 2 D shuffles -- was measured
+// and is slightly slower: second pass 0.197 -> 0.212 ms at 2^20 candidates, 0.104 -> 0.108 ms at 2^18.)
 // Every row is the same FMA chain as in rollout_reg_kernel (columns descending, first product a plain multiply), so states,
 // flags and keys are bit-identical to it: which lane computes a row does not change its bits.
 #pragma once
