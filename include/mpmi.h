@@ -54,7 +54,9 @@ enum { MPMI_DUMP_NONE = 0, MPMI_DUMP_PHYS = 1, MPMI_DUMP_LIFTED = 2 };
 enum { MPMI_MODEL_LINEAR = 0,   /* z' = K z + B u, lifted once, x = z[0:n] (north_star)        */
        MPMI_MODEL_RELIFT = 1 }; /* x' = C (K Psi(x) + B u): the physical state is re-lifted before every
                                    step, the literal f(x, u) on states of PAPER.md:132 (G18)     */
-/* mpmi_config.variant: results never depend on these, only speed does */
+/* mpmi_config.variant: speed knobs.  Flags and winner do not depend on them, with one documented exception: the latency
+ * kernel associates each row sum as two chains (csrc/rollout_lat.cuh), so a candidate within rounding of a boundary can
+ * differ between it and the other FP32 kernels (well inside tolerance T1). */
 enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)                  */
        MPMI_VARIANT_WIDE = 2,           /* 64/D candidates per thread (throughput)            */
        MPMI_VARIANT_NO_BINNING = 4,     /* never order the Philox candidates spatially        */
@@ -243,6 +245,27 @@ int mpmi_shard_finalize(mpmi_ctx *ctx, const mpmi_partial *d_partials, int32_t G
 int mpmi_rollout_batch(mpmi_ctx *ctx, const float *d_U, const float *d_X0, int64_t x0_count,
                        int64_t Ncand, int32_t H, int32_t dump_kind, float *d_traj,
                        int32_t *d_steps, uint8_t *d_safe, uint64_t tick, void *cuda_stream);
+
+/* One whole tick WITHOUT a context and without any allocation (csrc/noalloc.cu) -- for callers that may not call
+ * cudaMalloc: code under stream capture, tight serving loops, harnesses that forbid it.  The call enqueues two kernels on
+ * cuda_stream (model pack + the shared-memory-model register tick kernel, the FP32 path of Algorithm 2,
+ * PAPER.md:137-173) and returns; it calls no cudaMalloc / cudaFree / cudaHostAlloc, creates no graph, stream or event.
+ *   cfg       host struct as for mpmi_create, EXCEPT that the tables K (d*d), B (d*m), lift.terms (d*4, MONO), lift.W,
+ *             lift.b (RFF) are DEVICE pointers here (read by the kernels, not validated: the requirements of mpmi_create
+ *             on them are the caller's to keep); u_lo, u_hi, grid_counts, safe.idx / lo / hi stay host arrays, read
+ *             during the call.  variant is ignored.  Runs on the CURRENT device; cfg->device must be -1 or that device.
+ *   d_x0, d_u_user, d_out   device, as for mpmi_step_device; the result is the one mpmi_step_device gives for the same
+ *             configuration: bit-identical where that context runs the register kernel (info.variant == 1, e.g. with
+ *             MPMI_VARIANT_NARROW | MPMI_VARIANT_NO_TENSOR); against the latency kernel, whose row sums are associated
+ *             differently, a candidate within rounding of the boundary may differ, as between those two kernels.
+ * Limits: d <= 32 (the kernels' scratch -- the packed model and the cross-CTA selection state -- lives in ONE static
+ * 8 KB __device__ array per GPU, held until the process exits), linear model, noise_sigma == 0, the whole candidate set
+ * (shard 0,0).  Beyond them: MPMI_ERR_UNSUPPORTED, text in mpmi_noalloc_last_error (per host thread, valid until the
+ * next call).  Every call on a GPU shares that array and re-initialises it: calls whose kernels OVERLAP on the GPU
+ * (different streams, or several host threads) race on it -- serialise them.  Asynchronous. */
+int mpmi_tick_noalloc(const mpmi_config *cfg, const float *d_x0, const float *d_u_user, uint64_t tick,
+                      void *cuda_stream, mpmi_result *d_out);
+const char *mpmi_noalloc_last_error(void);
 
 int mpmi_get_info(const mpmi_ctx *ctx, mpmi_info *out);
 const char *mpmi_strerror(int status);

@@ -19,7 +19,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("MPMI_NVCC_EXTRA", "").split()     # e.g. -DMPMI_TC_DEBUG: in-kernel clock64 timelines
 
-UNITS = [("api", "mpmi_api.cu", [])]
+UNITS = [("api", "mpmi_api.cu", []), ("noalloc", "noalloc.cu", [])]
 UNITS += [(f"reg{d}_{m}", "inst_reg.cu", [f"-DMPMI_D={d}", f"-DMPMI_MODE={m}"]) for d in (32, 16, 8) for m in (0, 1)]
 UNITS += [(f"lat{d}", "inst_lat.cu", [f"-DMPMI_D={d}"]) for d in (32, 16, 8)]
 UNITS += [(f"regn{d}_{m}", "inst_reg.cu", [f"-DMPMI_D={d}", f"-DMPMI_MODE={m}", "-DMPMI_NOISE=1"]) for d in (32, 16, 8) for m in (0, 1)]

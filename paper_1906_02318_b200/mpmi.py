@@ -20,7 +20,7 @@ VARIANT_TENSOR32, VARIANT_SMEM_MODEL, VARIANT_TC_UNVERIFIED = 1024, 2048, 4096
 
 EXPORTS = ("mpmi_create", "mpmi_destroy", "mpmi_step", "mpmi_step_result", "mpmi_step_sync",
            "mpmi_step_device", "mpmi_step_trace", "mpmi_profile_enable", "mpmi_profile_timeline", "mpmi_profile_read", "mpmi_shard_step", "mpmi_shard_finalize", "mpmi_rollout_batch",
-           "mpmi_get_info", "mpmi_strerror", "mpmi_last_error")
+           "mpmi_get_info", "mpmi_strerror", "mpmi_last_error", "mpmi_tick_noalloc", "mpmi_noalloc_last_error")
 
 
 class MpmiError(RuntimeError):
@@ -109,6 +109,8 @@ def load_library():
     lib.mpmi_get_info.argtypes = [vp, C.POINTER(Info)]
     lib.mpmi_strerror.argtypes = [C.c_int]; lib.mpmi_strerror.restype = C.c_char_p
     lib.mpmi_last_error.argtypes = [vp]; lib.mpmi_last_error.restype = C.c_char_p
+    lib.mpmi_tick_noalloc.argtypes = [C.POINTER(_Config), vp, vp, u64, vp, vp]
+    lib.mpmi_noalloc_last_error.argtypes = []; lib.mpmi_noalloc_last_error.restype = C.c_char_p
     for name in EXPORTS:
         if getattr(lib, name).restype is C.c_int and name not in ("mpmi_destroy",):
             getattr(lib, name).restype = C.c_int
@@ -236,3 +238,31 @@ class Context:
     def rollout_batch(self, d_U, d_X0, x0_count, ncand, H, dump_kind, d_traj, d_steps, d_safe, tick=0, stream=0):
         self._check(self._lib.mpmi_rollout_batch(self._h, d_U, d_X0, int(x0_count), int(ncand), int(H), int(dump_kind),
                                                  d_traj, d_steps, d_safe, int(tick), stream))
+
+
+def tick_noalloc(w, d_K, d_B, d_x0, d_u_user, tick, stream, d_out, d_terms=None, d_W=None, d_b=None, N=None, H=None,
+                 include_user=None, device=-1):
+    """mpmi_tick_noalloc: one tick without a context and without any allocation in the library.  `w` carries the small
+    host-side fields of mpmi_config (as for Context); the tables are DEVICE pointers (ints): d_K (d*d), d_B (d*m),
+    d_terms (d*4 bytes, MONO lift) or d_W / d_b (RFF lift)."""
+    lib = load_library()
+    g = (lambda k, dflt=None: w[k] if isinstance(w, dict) and k in w else getattr(w, k, dflt))
+    keep = dict(u_lo=_f32(g("u_lo")), u_hi=_f32(g("u_hi")),
+                grid=None if g("grid_counts") is None else np.ascontiguousarray(g("grid_counts"), dtype=np.int32),
+                bidx=np.ascontiguousarray(g("bidx") if g("bidx") is not None else [], dtype=np.int32),
+                blo=_f32(g("blo", [])), bhi=_f32(g("bhi", [])))
+    c = _Config()
+    c.n, c.m, c.d = int(g("n")), int(g("m")), int(g("d"))
+    c.N, c.H = int(N if N is not None else g("N")), int(H if H is not None else g("H"))
+    c.K, c.B, c.u_lo, c.u_hi = d_K, d_B, _p(keep["u_lo"]), _p(keep["u_hi"])
+    c.sampler, c.grid_counts, c.seed = int(g("sampler", 0)), _p(keep["grid"]), int(g("seed", 0))
+    c.include_user = int(g("include_user", 1) if include_user is None else include_user)
+    c.lift = _Lift(int(g("lift_kind", 0)), d_terms, d_W, d_b, float(g("scale", 1.0)))
+    c.safe = _Safe(len(keep["bidx"]), _p(keep["bidx"]), _p(keep["blo"]), _p(keep["bhi"]),
+                   int(g("annulus", 0)), int(g("ix", 0)), int(g("iy", 1)), float(g("cx", 0.0)), float(g("cy", 0.0)),
+                   float(g("rmin", 0.0)), float(g("rmax", 0.0)), float(g("inflate", 0.0)))
+    c.device, c.shard_begin, c.shard_count, c.variant = device, 0, 0, 0
+    c.noise_sigma, c.model = float(g("noise_sigma", 0.0)), int(g("model_kind", 0))
+    rc = lib.mpmi_tick_noalloc(C.byref(c), d_x0, d_u_user, int(tick), stream, d_out)
+    if rc != OK:
+        raise MpmiError(rc, lib.mpmi_noalloc_last_error().decode() or lib.mpmi_strerror(rc).decode())

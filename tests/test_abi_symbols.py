@@ -16,7 +16,7 @@ def test_library_exports_every_declared_symbol():
     from paper_1906_02318_b200 import build
     lib = ctypes.CDLL(build.build())
     names = _declared()
-    assert len(names) == 16, names
+    assert len(names) == 18, names
     for name in names:
         assert hasattr(lib, name), name
 
