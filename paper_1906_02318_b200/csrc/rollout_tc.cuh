@@ -81,6 +81,17 @@ __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__flo
 // toward zero of ~2^-22 |x| per operand that adds up coherently over the horizon.  Adding half a TF32 ulp
 // to the bit pattern first turns the hardware's truncation into round-half-away (one integer add).
 __device__ __forceinline__ uint32_t tf32_lo(float x) { return __float_as_uint(x - tf32_hi(x)) + 0x1000u; }
+// the same for two values at once: the exact subtraction as one packed FADD2 (sub.rn.f32x2) -- per step and thread the split
+// is the bulk of the state warps' instructions (LOP3 + FADD + IADD per value), and four CTAs per SM share each scheduler
+__device__ __forceinline__ void tf32_lo2(uint32_t x0, uint32_t x1, uint32_t &l0, uint32_t &l1) {
+    const uint32_t h0 = x0 & 0xFFFFE000u, h1 = x1 & 0xFFFFE000u;
+    unsigned long long xx, hh, ll;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(xx) : "r"(x0), "r"(x1));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(hh) : "r"(h0), "r"(h1));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(ll) : "l"(xx), "l"(hh));
+    asm("mov.b64 {%0,%1}, %2;" : "=r"(l0), "=r"(l1) : "l"(ll));
+    l0 += 0x1000u; l1 += 0x1000u;
+}
 // round-to-nearest TF32 (ties away) and the matching low part x - x_hi (exact in fp32, either sign), itself rounded as above
 __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u); }
 __device__ __forceinline__ uint32_t tf32_lo_of(float x, float x_hi) { return __float_as_uint(x - x_hi) + 0x1000u; }
@@ -476,7 +487,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     for (int cc = 0; cc < kTcCols; cc += 8) {
                         uint32_t lo[8];
 #pragma unroll
-                        for (int j = 0; j < 8; j++) lo[j] = tf32_lo(__uint_as_float(r[cc + j]));
+                        for (int j = 0; j < 8; j += 2) tf32_lo2(r[cc + j], r[cc + j + 1], lo[j], lo[j + 1]);
                         tmem_st8(tlane + kTcColAlo + c0 + cc, lo);
                     }
                     if (NOISE && hc == kTcStateWarps / 4 - 1)      // noise of MMA step s (it produces z_{s+1})
