@@ -7,7 +7,8 @@
 // box they fall in (cell = the top bits of the Philox words, row-major over the input dimensions):
 //   bin_hist_kernel    histogram of cells (one RED per candidate) + exclusive scan by the last CTA
 //   bin_scatter_kernel perm[cursor[cell]++] = local candidate index
-//   bin_predict_kernel (life-time order, below) replaces bin_hist_kernel: keys + histogram + scan
+//   bin_predict_kernel (life-time order, below) replaces bin_hist_kernel: keys + histogram + scan;
+//   bin_scatter_keys_kernel is its scatter
 // The rollout kernel then walks perm, so a warp owns candidates of the same cell.  The candidate SET,
 // every key and hence the result are unchanged (keys carry the original index).
 // Life-time order (persistent tile kernels, d > 32): in a 3-D input box cubic cells leave a tile of 128 candidates
@@ -57,16 +58,23 @@ __device__ __forceinline__ void bin_scan_last_cta(const BinArgs &b) {
     __syncthreads();
     if (!last) return;
     __threadfence();
-    // exclusive scan of hist -> cursor by this (last) CTA; hist is cleared for the next tick
+    // exclusive scan of hist -> cursor by this (last) CTA; hist is cleared for the next tick.  64 consecutive cells per thread
+    // and pass as 16 int4 loads, all in flight at once: 16,384 cells are one L2 round trip (with 4 cells per thread the 16
+    // dependent passes were a serial tail of bin_hist_kernel on C4).  hist and cursor are allocated padded to a multiple of 64
+    // cells (mpmi_api.cu), the padding of hist stays zero.
+    constexpr int kScanCpt = 64;
     int carry = 0;
-    for (int base = 0; base < b.ncells; base += 256 * 4) {
-        int v[4], s = 0;
-        const int c0 = base + threadIdx.x * 4;
+    for (int base = 0; base < b.ncells; base += 256 * kScanCpt) {
+        int4 v[kScanCpt / 4];
+        int s = 0;
+        const int c0 = base + threadIdx.x * kScanCpt;
 #pragma unroll
-        for (int q = 0; q < 4; q++) {
-            v[q] = c0 + q < b.ncells ? __ldcg(&b.hist[c0 + q]) : 0;
-            if (c0 + q < b.ncells) b.hist[c0 + q] = 0;
-            s += v[q];
+        for (int q = 0; q < kScanCpt / 4; q++)
+            v[q] = c0 + 4 * q < b.ncells ? __ldcg(reinterpret_cast<const int4 *>(b.hist + c0) + q) : make_int4(0, 0, 0, 0);
+#pragma unroll
+        for (int q = 0; q < kScanCpt / 4; q++) {
+            if (c0 + 4 * q < b.ncells) reinterpret_cast<int4 *>(b.hist + c0)[q] = make_int4(0, 0, 0, 0);
+            s += v[q].x + v[q].y + v[q].z + v[q].w;
         }
         int incl = s;
 #pragma unroll
@@ -84,9 +92,13 @@ __device__ __forceinline__ void bin_scan_last_cta(const BinArgs &b) {
         }
         int run = carry + woff + incl - s;
 #pragma unroll
-        for (int q = 0; q < 4; q++) {
-            if (c0 + q < b.ncells) b.cursor[c0 + q] = run;
-            run += v[q];
+        for (int q = 0; q < kScanCpt / 4; q++) {
+            int4 o4;
+            o4.x = run; run += v[q].x;
+            o4.y = run; run += v[q].y;
+            o4.z = run; run += v[q].z;
+            o4.w = run; run += v[q].w;
+            if (c0 + 4 * q < b.ncells) reinterpret_cast<int4 *>(b.cursor + c0)[q] = o4;
         }
         carry += tot;
         __syncthreads();
@@ -109,76 +121,144 @@ __global__ void __launch_bounds__(256) bin_hist_kernel(const __grid_constant__ D
     bin_scan_last_cta(b);
 }
 
-// Life-time keys and their histogram in one pass: thread = candidate, x_k = a_k + G_k u from the [k][1 + m][NP] table
-// in shared memory (a_k: affine_base_kernel of this tick, G_k: mpmi_create), first violation -> keys[i]; then the same
-// last-CTA scan as bin_hist_kernel.  The warp leaves the horizon loop once all its candidates are predicted dead.
+// Life-time keys and their histogram in one pass: x_k = a_k + G_k u from the [k][1 + m][NP] table in shared memory (a_k:
+// affine_base_kernel of this tick, G_k: mpmi_create), first violation -> keys[i]; then the same last-CTA scan as
+// bin_hist_kernel.  A thread predicts kPredCand candidates: the table rows are warp-uniform LDS.128, each of which delivers
+// 512 B to the warp, and with one candidate per thread those loads alone were the kernel (78 us for C5's 262,144 candidates:
+// 8 LDS.128 per candidate-step = 32 clk of an SM's shared-memory bandwidth).  The life-time histogram is first built per CTA in
+// shared memory: the cell "survives the horizon" holds ~40 % of the candidates, and one global RED per warp on that one
+// address is serialised in L2.  Dynamic shared memory: the table, then H + 1 counters.
+constexpr int kPredCand = 4;
 template <int NP, int M>
 __global__ void __launch_bounds__(256) bin_predict_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
     static_assert(NP == 4 || NP == 8 || NP == 16, "padded physical dim");
     extern __shared__ __align__(16) float sag[];
     constexpr int stride = (1 + M) * NP;
+    constexpr int C = kPredCand;
     const int H = b.H;
+    int *s_hist = reinterpret_cast<int *>(sag + H * stride);
     for (int e = threadIdx.x; e < H * stride; e += 256) {
         const int k = e / stride, c = (e % stride) / NP, j = e % NP;
         sag[e] = c == 0 ? cfg.aff_a[k * NP + j] : cfg.aff_g[(k * M + (c - 1)) * NP + j];
     }
-    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    for (int e = threadIdx.x; e <= H; e += 256) s_hist[e] = 0;
+    const long long i0 = (long long)blockIdx.x * (256 * C) + threadIdx.x;
     const float none[kMaxM] = {0.f, 0.f, 0.f, 0.f};
-    float u[kMaxM];
-    sample_u(cfg, cfg.shard_begin + (i < b.nsamp ? i : 0), b.tick_val, none, u);
+    float u[C][kMaxM];
+    bool alive[C];
+    int steps[C];
+#pragma unroll
+    for (int c = 0; c < C; c++) {
+        const long long i = i0 + c * 256;
+        sample_u(cfg, cfg.shard_begin + (i < b.nsamp ? i : 0), b.tick_val, none, u[c]);
+        alive[c] = i < b.nsamp;
+        steps[c] = 0;
+    }
     // branch-free safe test: dims without a box limit hold (-inf, +inf) in cfg, no annulus becomes [0, +inf].  (An infinite
     // state in an unlimited dim is predicted unsafe here, the rollout kernels call it safe: the prediction only orders the walk.)
     const float r2lo = cfg.annulus ? cfg.rmin2 : 0.f, r2hi = cfg.annulus ? cfg.rmax2 : __int_as_float(0x7f800000);
     __syncthreads();
-    bool alive = i < b.nsamp;
-    int steps = 0;
-#pragma unroll 2
     for (int k = 0; k < H; k++) {
-        if (!__any_sync(0xffffffffu, alive)) break;
+        bool any = false;
+#pragma unroll
+        for (int c = 0; c < C; c++) any = any || alive[c];
+        if (!__any_sync(0xffffffffu, any)) break;
         const float4 *row = reinterpret_cast<const float4 *>(sag + k * stride);
-        float x[NP];
+        bool ok[C];
 #pragma unroll
-        for (int j = 0; j < NP / 4; j++) {
-            float4 v = row[j];
+        for (int c = 0; c < C; c++) ok[c] = alive[c];
 #pragma unroll
-            for (int q = 0; q < M; q++) {
-                const float4 g = row[(1 + q) * (NP / 4) + j];
-                v.x = __fmaf_rn(g.x, u[q], v.x); v.y = __fmaf_rn(g.y, u[q], v.y);
-                v.z = __fmaf_rn(g.z, u[q], v.z); v.w = __fmaf_rn(g.w, u[q], v.w);
+        for (int j = 0; j < NP / 4; j++) {                 // four physical dims at a time: the box test is separable
+            const float4 a4 = row[j];
+            float4 g4[M];
+#pragma unroll
+            for (int q = 0; q < M; q++) g4[q] = row[(1 + q) * (NP / 4) + j];
+#pragma unroll
+            for (int c = 0; c < C; c++) {
+                float4 v = a4;
+#pragma unroll
+                for (int q = 0; q < M; q++) {
+                    v.x = __fmaf_rn(g4[q].x, u[c][q], v.x); v.y = __fmaf_rn(g4[q].y, u[c][q], v.y);
+                    v.z = __fmaf_rn(g4[q].z, u[c][q], v.z); v.w = __fmaf_rn(g4[q].w, u[c][q], v.w);
+                }
+                if (j == 0) {
+                    const float dx = __fsub_rn(v.x, cfg.cx), dy = __fsub_rn(v.y, cfg.cy);
+                    const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
+                    ok[c] = ok[c] && (r2 >= r2lo) && (r2 <= r2hi);
+                }
+                ok[c] = ok[c] && (v.x > cfg.blo[4 * j]) && (v.x < cfg.bhi[4 * j]) && (v.y > cfg.blo[4 * j + 1]) && (v.y < cfg.bhi[4 * j + 1]) &&
+                        (v.z > cfg.blo[4 * j + 2]) && (v.z < cfg.bhi[4 * j + 2]) && (v.w > cfg.blo[4 * j + 3]) && (v.w < cfg.bhi[4 * j + 3]);
             }
-            x[4 * j] = v.x; x[4 * j + 1] = v.y; x[4 * j + 2] = v.z; x[4 * j + 3] = v.w;
         }
-        const float dx = __fsub_rn(x[0], cfg.cx), dy = __fsub_rn(x[1], cfg.cy);
-        const float r2 = __fmaf_rn(dx, dx, __fmul_rn(dy, dy));
-        bool ok = alive && (r2 >= r2lo) && (r2 <= r2hi);
 #pragma unroll
-        for (int j = 0; j < NP; j++) ok = ok && (x[j] > cfg.blo[j]) && (x[j] < cfg.bhi[j]);
-        alive = ok;
-        steps += alive ? 1 : 0;
+        for (int c = 0; c < C; c++) { alive[c] = ok[c]; steps[c] += ok[c] ? 1 : 0; }
     }
-    if (i < b.nsamp) {
-        b.keys[i] = steps;
-        const int cell = H - steps;
-        const unsigned peers = __match_any_sync(__activemask(), cell);
-        if ((threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&b.hist[cell], __popc(peers));
+#pragma unroll
+    for (int c = 0; c < C; c++) {
+        const long long i = i0 + c * 256;
+        if (i < b.nsamp) {
+            b.keys[i] = steps[c];
+            const int cell = H - steps[c];
+            const unsigned peers = __match_any_sync(__activemask(), cell);
+            if ((threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&s_hist[cell], __popc(peers));
+        }
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e <= H; e += 256) {
+        const int v = s_hist[e];
+        if (v) atomicAdd(&b.hist[e], v);
     }
     bin_scan_last_cta(b);
 }
 
+// cells from the Philox words (uniform over the cells: no contention; four candidates per thread and pass with their
+// fetch-and-adds in flight together were measured slower: 20.2 against 18.3 us for 2^20 candidates)
 __global__ void __launch_bounds__(256) bin_scatter_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
     const unsigned long long tick = b.tick_val;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < b.nsamp; i += (long long)gridDim.x * blockDim.x) {
         const int cell = cell_of(cfg, b, cfg.shard_begin + i, tick);
-        int pos = 0;
-        if (b.keys) {
-            const unsigned peers = __match_any_sync(__activemask(), cell);
-            const int lead = __ffs(peers) - 1, lane = threadIdx.x & 31;
-            if (lane == lead) pos = atomicAdd(&b.cursor[cell], __popc(peers));
-            pos = __shfl_sync(peers, pos, lead) + __popc(peers & ((1u << lane) - 1u));
-        } else {
-            pos = atomicAdd(&b.cursor[cell], 1);
+        b.perm[atomicAdd(&b.cursor[cell], 1)] = (int)i;
+    }
+}
+
+// life-time order: few cells, one of them holding ~40 % of the candidates.  A CTA ranks its 1,024 candidates per cell in shared
+// memory and takes ONE global fetch-and-add per cell it holds (with one per warp and cell the hot cell's 8,192 same-address
+// atomics were the kernel: 18 us for 262,144 candidates).  Dynamic shared memory: 2 * ncells ints.
+__global__ void __launch_bounds__(256) bin_scatter_keys_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ BinArgs b) {
+    constexpr int C = 4;
+    extern __shared__ int s_bin[];
+    int *s_cnt = s_bin, *s_base = s_bin + b.ncells;
+    const int lane = threadIdx.x & 31;
+    for (long long chunk = blockIdx.x; chunk * (256 * C) < b.nsamp; chunk += gridDim.x) {
+        for (int e = threadIdx.x; e < b.ncells; e += 256) s_cnt[e] = 0;
+        __syncthreads();
+        int cell[C], rank[C];
+#pragma unroll
+        for (int c = 0; c < C; c++) {
+            const long long i = chunk * (256 * C) + c * 256 + threadIdx.x;
+            cell[c] = 0; rank[c] = 0;
+            if (i < b.nsamp) {
+                const int st = b.keys[i];
+                cell[c] = b.H - (st < 0 ? 0 : st > b.H ? b.H : st);
+                const unsigned peers = __match_any_sync(__activemask(), cell[c]);
+                const int lead = __ffs(peers) - 1;
+                int pos = 0;
+                if (lane == lead) pos = atomicAdd(&s_cnt[cell[c]], __popc(peers));
+                rank[c] = __shfl_sync(peers, pos, lead) + __popc(peers & ((1u << lane) - 1u));
+            }
         }
-        b.perm[pos] = (int)i;
+        __syncthreads();
+        for (int e = threadIdx.x; e < b.ncells; e += 256) {
+            const int v = s_cnt[e];
+            if (v) s_base[e] = atomicAdd(&b.cursor[e], v);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < C; c++) {
+            const long long i = chunk * (256 * C) + c * 256 + threadIdx.x;
+            if (i < b.nsamp) b.perm[s_base[cell[c]] + rank[c]] = (int)i;
+        }
+        __syncthreads();
     }
 }
 

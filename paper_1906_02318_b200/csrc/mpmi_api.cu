@@ -261,7 +261,16 @@ const void *pick_predict_m(int m) {
          : m == 3 ? (const void *)bin_predict_kernel<NP, 3> : (const void *)bin_predict_kernel<NP, 4>;
 }
 const void *pick_predict(int np, int m) { return np == 4 ? pick_predict_m<4>(m) : np == 8 ? pick_predict_m<8>(m) : pick_predict_m<16>(m); }
-unsigned pred_smem(const mpmi_ctx *c) { return (unsigned)(c->dc.H * (1 + c->dc.m) * c->dc.aff_np * 4); }
+unsigned pred_smem(const mpmi_ctx *c) { return (unsigned)(c->dc.H * (1 + c->dc.m) * c->dc.aff_np * 4 + (c->dc.H + 1) * 4); }   // table + CTA histogram
+unsigned pred_grid(const mpmi_ctx *c) { return (unsigned)((c->bin.nsamp + 256 * kPredCand - 1) / (256 * kPredCand)); }
+// scatter of the binning pass: cells from the Philox words, or (life-time order) from the predicted keys
+const void *scatter_fn(const mpmi_ctx *c) { return c->predict ? (const void *)bin_scatter_keys_kernel : (const void *)bin_scatter_kernel; }
+unsigned scatter_smem(const mpmi_ctx *c) { return c->predict ? (unsigned)(2 * c->bin.ncells * sizeof(int)) : 0u; }
+unsigned scatter_grid(const mpmi_ctx *c, unsigned bin_grid) {
+    if (!c->predict) return bin_grid;
+    const long long g = (c->bin.nsamp + 1023) / 1024, gmax = 8LL * c->sm_count;
+    return (unsigned)(g < gmax ? g : gmax);
+}
 
 #define CL(call) do { const cudaError_t e_ = (call); if (e_ != cudaSuccess) return e_; } while (0)
 // bound kernels of the verified tensor-core tick (bound.cuh): E[j][r] for this x_t, then tau_i(k)
@@ -304,11 +313,11 @@ cudaError_t enqueue_tick(const mpmi_ctx *c, KArgs a, cudaStream_t s) {
         void *pargs[2] = {(void *)&c->dc, (void *)&b};
         if (c->predict) {        // a_k for this x_t, then predicted life times (keys) + their histogram + scan
             CL(launch_base(c, a, s));
-            CL(cudaLaunchKernel(c->k_pred, dim3((unsigned)g), dim3(256), pargs, pred_smem(c), s));
+            CL(cudaLaunchKernel(c->k_pred, dim3(pred_grid(c)), dim3(256), pargs, pred_smem(c), s));
         } else {
             CL(cudaLaunchKernel((const void *)bin_hist_kernel, dim3(grid), dim3(256), pargs, 0, s));
         }
-        CL(cudaLaunchKernel((const void *)bin_scatter_kernel, dim3(grid), dim3(256), pargs, 0, s));
+        CL(cudaLaunchKernel(scatter_fn(c), dim3(scatter_grid(c, grid)), dim3(256), pargs, scatter_smem(c), s));
         a.perm = c->d_perm; a.nsamp = b.nsamp;
     }
     if (c->affine) CL(launch_base(c, a, s));
@@ -348,14 +357,15 @@ void base_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
 void pred_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
     args[0] = (void *)&c->dc; args[1] = (void *)&c->gb;
-    p->func = (void *)c->k_pred; p->gridDim = dim3((unsigned)((c->bin.nsamp + 255) / 256)); p->blockDim = dim3(256);
+    p->func = (void *)c->k_pred; p->gridDim = dim3(pred_grid(c)); p->blockDim = dim3(256);
     p->sharedMemBytes = pred_smem(c); p->kernelParams = args;
 }
 void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **args) {
     std::memset(p, 0, sizeof *p);
     args[0] = (void *)&c->dc; args[1] = (void *)&c->gb;
-    p->func = scatter ? (void *)bin_scatter_kernel : (void *)bin_hist_kernel;
-    p->gridDim = dim3(c->bin_grid); p->blockDim = dim3(256); p->kernelParams = args;
+    p->func = scatter ? (void *)scatter_fn(c) : (void *)bin_hist_kernel;
+    p->gridDim = dim3(scatter ? scatter_grid(c, c->bin_grid) : c->bin_grid); p->blockDim = dim3(256); p->kernelParams = args;
+    p->sharedMemBytes = scatter ? scatter_smem(c) : 0u;
 }
 
 void recheck_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
@@ -648,10 +658,12 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             for (int t = 0; t < total; t++) c->bin.bits[t % m]++;
             c->bin.ncells = 1 << total;
             c->bin.nsamp = nsamp;
-            const size_t ncell_alloc = (size_t)(c->bin.ncells > cfg->H + 1 ? c->bin.ncells : cfg->H + 1);   // (life-time order: H + 1 cells)
+            // (life-time order: H + 1 cells; padded to whole 64-cell groups for the scan's int4 accesses, the padding stays zero)
+            const size_t ncell_alloc = (((size_t)(c->bin.ncells > cfg->H + 1 ? c->bin.ncells : cfg->H + 1) + 63) / 64) * 64;
             CUC(cudaMalloc(&c->d_hist, sizeof(int) * ncell_alloc));
             CUC(cudaMemset(c->d_hist, 0, sizeof(int) * ncell_alloc));
             CUC(cudaMalloc(&c->d_cursor, sizeof(int) * ncell_alloc));
+            CUC(cudaMemset(c->d_cursor, 0, sizeof(int) * ncell_alloc));
             CUC(cudaMalloc(&c->d_perm, sizeof(int) * nsamp));
             CUC(cudaMalloc(&c->d_bin_ticket, sizeof(unsigned)));
             CUC(cudaMemset(c->d_bin_ticket, 0, sizeof(unsigned)));
@@ -816,7 +828,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         CUC(cudaMalloc(&c->d_pred, sizeof(int) * c->bin.nsamp));
         c->predict = true;
         c->k_pred = pick_predict(NPn, m);
-        CUC(cudaFuncSetAttribute(c->k_pred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem));
+        CUC(cudaFuncSetAttribute(c->k_pred, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aff_smem + (cfg->H + 1) * 4));
         c->bin.keys = c->d_pred; c->bin.H = cfg->H; c->bin.ncells = cfg->H + 1;
     }
     // ---- verified tensor-core tick: second-pass kernel, deferral lists, bound tables (bound.cuh) -----------------------------
