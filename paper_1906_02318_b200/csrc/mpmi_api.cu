@@ -82,6 +82,7 @@ struct mpmi_ctx {
     unsigned recheck_grid = 0;
     int recheck_block = kRegBlock, recheck_smem = 0, fp32_smem = 0;
     bool recheck_persistent = false;
+    int rc_warps = 0;                // MPMI_RC_WARPS (measurement): active warps per CTA of the d = 128 second pass
     float recheck_tau_scale = 1.f;   // MPMI_TC_TAU_SCALE (measures how conservative the bound is; not a tuning knob)
     cudaGraphNode_t n_recheck = nullptr, n_berr = nullptr, n_btau = nullptr;
     const void *k_berr = nullptr, *k_btau = nullptr;
@@ -285,7 +286,7 @@ cudaError_t launch_bound(const mpmi_ctx *c, const KArgs &a, cudaStream_t s) {
 }
 // second pass of the verified tick / batch: the FP32 kernel over the deferral lists
 cudaError_t launch_recheck(const mpmi_ctx *c, KernFn fn, KArgs a, cudaStream_t s) {
-    a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1; a.kslot = c->kslot; a.st = c->d_state;
+    a.perm = nullptr; a.nsamp = 0; a.recheck_mode = 1 | (c->rc_warps << 8); a.kslot = c->kslot; a.st = c->d_state;
     a.work = c->recheck_persistent ? &c->d_state->work : nullptr;
     void *args[2] = {(void *)&c->dc, (void *)&a};
     return cudaLaunchKernel((const void *)fn, dim3(c->recheck_grid), dim3((unsigned)c->recheck_block), args, (size_t)c->recheck_smem, s);
@@ -370,7 +371,7 @@ void bin_node_params(mpmi_ctx *c, bool scatter, cudaKernelNodeParams *p, void **
 
 void recheck_node_params(mpmi_ctx *c, cudaKernelNodeParams *p, void **args) {
     c->gr = c->ga;                               // same inputs, sequence number and result slot as the tick node
-    c->gr.perm = nullptr; c->gr.nsamp = 0; c->gr.recheck_mode = 1;
+    c->gr.perm = nullptr; c->gr.nsamp = 0; c->gr.recheck_mode = 1 | (c->rc_warps << 8);
     c->gr.work = c->recheck_persistent ? &c->d_state->work : nullptr;
     std::memset(p, 0, sizeof *p);
     args[0] = (void *)&c->dc; args[1] = (void *)&c->gr;
@@ -552,6 +553,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
     mpmi_ctx *c = new (std::nothrow) mpmi_ctx();
     if (!c) return fail(nullptr, MPMI_ERR_NOMEM, "host allocation failed");
     c->device = dev;
+    if (const char *e = std::getenv("MPMI_RC_WARPS")) c->rc_warps = std::atoi(e) & 31;
     c->sm_count = prop.multiProcessorCount;
     int rc = MPMI_OK;
     auto bail = [&](int code) { g_create_err = c->err; mpmi_destroy(c); return code; };

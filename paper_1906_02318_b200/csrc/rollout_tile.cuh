@@ -22,26 +22,30 @@ constexpr int kTileWC = 16;                      // candidates per warp batch (1
 constexpr int kTileWarps = kTileNC / kTileWC;
 constexpr int kTileThreadsT = kTileWarps * 32;
 
-constexpr int kTileWCRecheck = 8;                // second pass of the verified tensor-core tick: 8 candidates per warp batch
+#ifndef MPMI_TILE_WC_RECHECK
+#define MPMI_TILE_WC_RECHECK 4
+#endif
+constexpr int kTileWCRecheck = MPMI_TILE_WC_RECHECK;   // second pass of the verified tensor-core tick: candidates per warp batch
 
 template <int D, int M, int WCP = kTileWC>
 constexpr int tile_smem_bytes() { return ((D + M) * D + kTileWarps * (D + M) * WCP) * 4; }
 
 // WCP = candidates per warp batch.  16 for whole ticks (lane = 8 rows x 8 candidates).  The second pass of the verified
 // tensor-core tick (kernel_args.cuh: recheck) sees a few per cent of the candidates -- fewer warp batches than the machine
-// has warps -- so there the batch is 8 candidates (lane = 4 rows x 8 candidates) and batches are dealt out statically,
-// longest-lived first, round-robin over CTAs and then over the warps of a CTA: every SM sub-partition gets the same number
-// of batches, a long, a medium and a short one (measured with 16-candidate batches fetched first-come: 1.3 ms for 5 % of
-// C5's candidates, some sub-partitions holding four full-horizon batches).  Same FMA chain per (row, candidate), hence the
-// same bits, for either batch size.
+// has warps -- and lasts as long as its full-horizon batches: there the batch is 4 candidates (lane = 4 rows x 4 candidates),
+// which quarters that chain, and four warps per CTA fetch batches longest first (see the batch loop).  Same FMA chain per
+// (row, candidate), hence the same bits, for every batch size.
 template <int D, int M, int MODE, bool NOISE = false, int WCP = kTileWC>
 __global__ void __launch_bounds__(kTileThreadsT, 1)
 rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
     constexpr int WC = WCP;
-    constexpr int CG = WC / 8;                    // candidate groups per warp: every lane owns 8 candidates
+    constexpr int CL = WC < 8 ? WC : 8;           // candidates per lane (8; 4 for 4-candidate batches)
+    constexpr int CG = WC / CL;                   // candidate groups per warp
     constexpr int RG = 32 / CG;                   // row groups per warp
     constexpr int TR = D / RG;                    // rows per lane
     constexpr int QR = TR / 4;                    // float4 groups of rows per lane
+    constexpr int NZ = CL / 4;                    // float4 groups of candidates per lane
+    static_assert(CL == 4 || CL == 8, "lane tile: 4 or 8 candidates");
     constexpr int kTileThreads = kTileThreadsT;
     static_assert(TR % 4 == 0, "lane tile");
     static_assert(D == 64 || D == 128, "tile kernel: D in {64, 128}");
@@ -93,18 +97,20 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
 
     for (long long round = 0;; round++) {
         // ---- next batch of WC candidates for this warp (dynamic: warps that exit early take more).
-        // Second pass: the lists are sorted longest-lived first and most deferred candidates are short-lived, so the pass lasts as
-        // long as a full-horizon batch needs on its SM sub-partition.  The 4 * gridDim longest batches are dealt out statically, one
-        // per sub-partition (warp w of a CTA runs on sub-partition w % 4), the longest ones to sub-partition 0 -- which is then left
-        // alone: warps 4, 8, 12 stay idle -- and every other batch is fetched first come, first served by the remaining warps.
-        // (Measured on C5, 4.8 % of the candidates: all batches first-come 1.3 ms; all dealt out statically 0.52 ms; static head +
-        // first-come tail with all 16 warps 0.57 ms; with sub-partition 0 left to the head batch 0.49 ms.)
-        if (rc && warp >= 4 && (warp & 3) == 0) break;
-        const bool fixed = rc && round == 0 && warp < 4;
+        // Second pass: the lists are sorted longest-lived first and most deferred candidates are short-lived.  Only FOUR warps of
+        // the CTA work, one per SM sub-partition (with the 16-fold unrolled column loop one warp keeps its sub-partition's FMA pipe
+        // busy; more warps only stretch the full-horizon batches, which set the length of the pass), each starting with one of
+        // the 4 * gridDim longest batches and fetching every further one first come, first served -- longest processing time first.
+        // (Measured on C5, 4.8 % of the candidates.  8-candidate batches: all 16 warps first-come 1.3 ms; all dealt out statically
+        // 0.52 ms; static head + first-come tail, sub-partition 0 left to its head batch, 13 warps 0.37 ms.  4-candidate batches,
+        // which halve a full-horizon batch's chain: 13 warps 0.33 ms; 16 / 12 / 8 / 4 warps first-come 0.31 / 0.30 / 0.28 / 0.275 ms.)
+        const int rc_warps = (a.recheck_mode >> 8) ? (a.recheck_mode >> 8) : 4;     // (MPMI_RC_WARPS: measurement)
+        if (rc && warp >= rc_warps) break;
+        const bool fixed = rc && round == 0;
         if (lane == 0) s_batch[warp] = fixed ? 0u : atomicAdd(a.work, 1u);
         __syncwarp();
         const long long batch = fixed ? (long long)blockIdx.x + (long long)gridDim.x * warp
-                                      : (long long)s_batch[warp] + (rc ? 4LL * gridDim.x : 0LL);
+                                      : (long long)s_batch[warp] + (rc ? (long long)rc_warps * gridDim.x : 0LL);
         __syncwarp();
         if (batch >= nbatch) break;
 
@@ -152,15 +158,15 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
         for (; k < H; k++) {
             if (!__any_sync(0xffffffffu, alive)) break;
 
-            float2 acc[TR][4];
+            float2 acc[TR][CL / 2];
 #pragma unroll
             for (int r = 0; r < TR; r++)
 #pragma unroll
-                for (int q = 0; q < 4; q++) acc[r][q] = make_float2(0.f, 0.f);
+                for (int q = 0; q < CL / 2; q++) acc[r][q] = make_float2(0.f, 0.f);
 
             // (second pass, WC = 8: few warps per sub-partition, so the shared-memory loads of the next columns must be in flight
             // under the FFMA2s of this one: deeper unrolling.  Measured on C5: unroll 2 / 8 / 16 / 32 -> 0.49 / 0.40 / 0.37 / 0.36 ms)
-#pragma unroll (WC == kTileWCRecheck ? 16 : 2)
+#pragma unroll (WC <= 8 ? 16 : 2)
             for (int cc = 0; cc < D + M; cc++) {                // descending column order: see rollout_reg.cuh
                 const int c = D + M - 1 - cc;
                 float kr[TR];
@@ -169,9 +175,9 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
                     const float4 v = *reinterpret_cast<const float4 *>(kp + c * D + q * (4 * RG));
                     kr[4 * q] = v.x; kr[4 * q + 1] = v.y; kr[4 * q + 2] = v.z; kr[4 * q + 3] = v.w;
                 }
-                float2 zc[4];
+                float2 zc[CL / 2];
 #pragma unroll
-                for (int q = 0; q < 2; q++) {
+                for (int q = 0; q < NZ; q++) {
                     const float4 v = *reinterpret_cast<const float4 *>(zp + c * WC + q * (4 * CG));
                     zc[2 * q] = make_float2(v.x, v.y);
                     zc[2 * q + 1] = make_float2(v.z, v.w);
@@ -179,14 +185,14 @@ rollout_tile_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ 
 #pragma unroll
                 for (int r = 0; r < TR; r++)
 #pragma unroll
-                    for (int q = 0; q < 4; q++) fma2_bcast(acc[r][q], kr[r], zc[q]);
+                    for (int q = 0; q < CL / 2; q++) fma2_bcast(acc[r][q], kr[r], zc[q]);
             }
             __syncwarp();                                  // every lane has finished reading Zw
 #pragma unroll
             for (int r = 0; r < TR; r++) {
                 const int row = (r >> 2) * (4 * RG) + rg * 4 + (r & 3);
 #pragma unroll
-                for (int q = 0; q < 2; q++)
+                for (int q = 0; q < NZ; q++)
                     *reinterpret_cast<float4 *>(zw + row * WC + q * (4 * CG) + cg * 4) =
                         make_float4(acc[r][2 * q].x, acc[r][2 * q].y, acc[r][2 * q + 1].x, acc[r][2 * q + 1].y);
             }
