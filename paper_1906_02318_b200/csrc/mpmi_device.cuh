@@ -330,6 +330,14 @@ __device__ __forceinline__ void fma2_bcast_z(float2 &acc, const float2 &k, float
     asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(aa) : "l"(kk), "l"(zz));
     asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
 }
+// acc = kpair * z (first column of a step, row-pair form)
+__device__ __forceinline__ void mul2_bcast_z(float2 &acc, const float2 &k, float z) {
+    unsigned long long kk, zz, aa;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(kk) : "f"(k.x), "f"(k.y));
+    asm("mov.b64 %0, {%1,%1};" : "=l"(zz) : "f"(z));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(aa) : "l"(kk), "l"(zz));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(aa));
+}
 // acc = k * z (first column of a step)
 __device__ __forceinline__ void mul2_bcast(float2 &acc, float k, const float2 &z) {
     unsigned long long kk, zz, aa;

@@ -15,6 +15,9 @@
 // 241 / 321 / 452 / 760 us with RS = 4; at 2^20 (40,000 deferred: throughput-bound again) 1.32 ms against 1.30 ms with RS = 2.
 // (An all-gather through shared memory -- RL / 2 STS.128 + D / 2 LDS.128 per lane instead of 2 D shuffles -- was measured
 // and is slightly slower: second pass 0.197 -> 0.212 ms at 2^20 candidates, 0.104 -> 0.108 ms at 2^18.)
+// (Round-2 late: FFMA2 over two ROWS of one candidate instead of one row of two candidates removed ~1.5 register moves per FFMA2
+// -- the pass was bound by issue slots: second pass at 2^20 candidates 0.198 -> 0.166 ms, verified tick at 2^16 .. 2^20 now
+// 208 / 263 / 376 / 596 / 964 us.)
 // Every row is the same FMA chain as in rollout_reg_kernel (columns descending, first product a plain multiply), so states,
 // flags and keys are bit-identical to it: which lane computes a row does not change its bits.
 #pragma once
@@ -88,7 +91,11 @@ rollout_split_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__
         // ---- a3 + a4: horizon loop
         for (int k = 0; k < H; k++) {
             if (!__any_sync(0xffffffffu, alive[0] || alive[1])) break;
-            float2 acc[RL];
+            // FFMA2 over two ROWS of one candidate (model pair straight from the LDS.128, state value broadcast): with the model
+            // value as the broadcast operand every FFMA2 needed its own {k, k} register pair -- ~1.5 moves per FFMA2, and the
+            // pass was bound by issue slots (two such warps per sub-partition), not by the FMA pipe.  The state value's pair
+            // is built once per column and candidate.  Same fma(k, z, acc) sequence per row as before: same bits.
+            float2 acc0[RL / 2], acc1[RL / 2];                   // candidate 0 / 1 of the pair, rows (2i, 2i + 1) of this lane
 #pragma unroll
             for (int cc = 0; cc < D + M; cc++) {                 // columns descending, as in rollout_reg_kernel
                 const int c = D + M - 1 - cc;
@@ -96,12 +103,13 @@ rollout_split_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__
 #pragma unroll
                 for (int r = 0; r < RL; r += 4) {
                     const float4 kv = lds128(sbase + (c * D + r) * 4);
+                    const float2 k01 = make_float2(kv.x, kv.y), k23 = make_float2(kv.z, kv.w);
                     if (cc == 0) {
-                        mul2_bcast(acc[r + 0], kv.x, zc); mul2_bcast(acc[r + 1], kv.y, zc);
-                        mul2_bcast(acc[r + 2], kv.z, zc); mul2_bcast(acc[r + 3], kv.w, zc);
+                        mul2_bcast_z(acc0[r / 2], k01, zc.x); mul2_bcast_z(acc0[r / 2 + 1], k23, zc.x);
+                        mul2_bcast_z(acc1[r / 2], k01, zc.y); mul2_bcast_z(acc1[r / 2 + 1], k23, zc.y);
                     } else {
-                        fma2_bcast(acc[r + 0], kv.x, zc); fma2_bcast(acc[r + 1], kv.y, zc);
-                        fma2_bcast(acc[r + 2], kv.z, zc); fma2_bcast(acc[r + 3], kv.w, zc);
+                        fma2_bcast_z(acc0[r / 2], k01, zc.x); fma2_bcast_z(acc0[r / 2 + 1], k23, zc.x);
+                        fma2_bcast_z(acc1[r / 2], k01, zc.y); fma2_bcast_z(acc1[r / 2 + 1], k23, zc.y);
                     }
                 }
             }
@@ -110,8 +118,8 @@ rollout_split_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__
             for (int qq = 0; qq < RS; qq++)
 #pragma unroll
                 for (int r = 0; r < RL; r++) {
-                    z[qq * RL + r].x = __shfl_sync(0xffffffffu, acc[r].x, qq, RS);
-                    z[qq * RL + r].y = __shfl_sync(0xffffffffu, acc[r].y, qq, RS);
+                    z[qq * RL + r].x = __shfl_sync(0xffffffffu, (r & 1) ? acc0[r / 2].y : acc0[r / 2].x, qq, RS);
+                    z[qq * RL + r].y = __shfl_sync(0xffffffffu, (r & 1) ? acc1[r / 2].y : acc1[r / 2].x, qq, RS);
                 }
             if (NOISE) {
                 // Algorithm 2 l.5: + z_i on the physical rows, before isSafe (every lane of the group draws the same eps)
