@@ -73,6 +73,7 @@ struct mpmi_ctx {
     int *d_pred = nullptr;
     const void *k_pred = nullptr;    // bin_predict_kernel<aff_np>
     int tc_ctas = 1;                 // persistent CTAs per SM (4 for the tensor-core kernel at D = 32)
+    long long lat_cap = 0;           // latency kernel: CTAs resident at once (its grid never exceeds them: rollout_lat.cuh)
     // verified tensor-core tick: the tcgen05 kernel defers the candidates that came within tau_i(k) (bound.cuh) of the
     // safe-set boundary to the FP32 kernel (register kernel at D = 32, warp-tile kernel at D = 128), which merges them and
     // finalises (kernel_args.cuh: recheck).  tau comes per tick from bound_err_kernel -> bound_tau_kernel.
@@ -234,6 +235,7 @@ cudaError_t launch_geom(const mpmi_ctx *c, KernFn fn, long long ncand, const KAr
                         bool persistent) {
     long long blocks = (ncand + cpb - 1) / cpb;
     if (blocks < 1) blocks = 1;
+    if (fn == c->k_tick && c->variant == 3 && c->lat_cap > 0 && blocks > c->lat_cap) blocks = c->lat_cap;
     KArgs a = a0;
     if (persistent) {                            // persistent warp-tile / tensor-core kernel: one CTA per SM
         if (blocks > (long long)c->sm_count * c->tc_ctas) blocks = (long long)c->sm_count * c->tc_ctas;
@@ -341,6 +343,7 @@ unsigned grid_for(const mpmi_ctx *c, long long ncand) {
     long long blocks = (ncand + c->cand_per_block - 1) / c->cand_per_block;
     if (blocks < 1) blocks = 1;
     if ((c->variant == 2 || c->variant == 4) && blocks > (long long)c->sm_count * c->tc_ctas) blocks = (long long)c->sm_count * c->tc_ctas;
+    if (c->variant == 3 && c->lat_cap > 0 && blocks > c->lat_cap) blocks = c->lat_cap;
     return (unsigned)blocks;
 }
 
@@ -717,6 +720,9 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             c->variant = 3;
             c->k_tick = pick_lat(D, M, R);
             c->block = 64; c->cand_per_block = 64 / (D / R);     // D/R lanes per candidate
+            int occ = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)c->k_tick, 64, 0) == cudaSuccess && occ > 0 && !std::getenv("MPMI_LAT_WAVES"))
+                c->lat_cap = (long long)occ * c->sm_count;
         }
         // D = 32, large candidate sets: the 3xTF32 tcgen05 kernel of d = 128 with N = 32 MMAs and four CTAs per SM, as a
         // VERIFIED tick (below).  The batch entry stays on the FP32 register kernels chosen above.

@@ -52,8 +52,27 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
     __syncthreads();
     MPMI_STAMP(2);                                // lift done, CTA synchronised
 
+    const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
+    const bool no_annulus = cfg.annulus == 0;
+    // only constrained dims are tested (as in every other kernel and in the oracle): an unconstrained dim passes whatever
+    // it holds, Inf and NaN included -- its (-inf, +inf) limits alone would reject those.  One AND per dim: the state's bit
+    // pattern is masked to +0.0 where the dim is unconstrained, and 0 lies inside (-inf, +inf).
+    unsigned zm[NB];
+#pragma unroll
+    for (int j = 0; j < NB; j++) zm[j] = ((cfg.bmask >> j) & 1u) ? 0xFFFFFFFFu : 0u;
+    unsigned long long key = kKeyNone;
+    unsigned n_safe = 0, n_exec = 0;
+
+    // A CTA rolls batches blockIdx, blockIdx + gridDim, ... of kLatBlock / L candidates.  The grid is one batch per CTA unless
+    // that exceeds what is resident at once (d = 32 with 4 rows per lane: 200 registers, i.e. two warps per sub-partition's 16 K
+    // registers, 4 CTAs per SM; 10,000 candidates are 1,251 batches): then the grid is the resident set, and a CTA's later batches
+    // re-use its model rows and its lift instead of paying the prologue again in another wave (mpmi_api.cu: lat_cap).  Measured:
+    // C4 model at 2^14 candidates 131 -> 121 us, C3 46.7 -> 45.2 us.  (Three warps per sub-partition need <= 168 registers: spills,
+    // 58 us at 176.)
+    const long long nbatch = (ncand + kLatBlock / L - 1) / (kLatBlock / L);
+  for (long long blk = blockIdx.x; blk < nbatch; blk += gridDim.x) {
     // ---- a1 + a2 ----------------------------------------------------------------------------------
-    const long long li = (long long)blockIdx.x * (kLatBlock / L) + tid / L;
+    const long long li = blk * (kLatBlock / L) + tid / L;
     bool alive = li < ncand && inputs_ok;
     int steps = 0;
     float z[D + M];
@@ -65,15 +84,7 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
 #pragma unroll
         for (int c = 0; c < D; c++) z[c] = sz0[c];
     }
-    MPMI_STAMP(3);                                // candidate sampled (Philox / grid), state initialised
-    const int nbox = __popc(cfg.bmask) ? 32 - __clz(cfg.bmask) : 0;
-    const bool no_annulus = cfg.annulus == 0;
-    // only constrained dims are tested (as in every other kernel and in the oracle): an unconstrained dim passes whatever
-    // it holds, Inf and NaN included -- its (-inf, +inf) limits alone would reject those.  One AND per dim: the state's bit
-    // pattern is masked to +0.0 where the dim is unconstrained, and 0 lies inside (-inf, +inf).
-    unsigned zm[NB];
-#pragma unroll
-    for (int j = 0; j < NB; j++) zm[j] = ((cfg.bmask >> j) & 1u) ? 0xFFFFFFFFu : 0u;
+    if (blk == blockIdx.x) MPMI_STAMP(3);         // candidate sampled (Philox / grid), state initialised (first batch)
 
     // ---- a3 + a4: no memory traffic inside this loop -----------------------------------------------
     for (int k = 0; k < H; k++) {
@@ -121,10 +132,8 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
         steps += alive ? 1 : 0;
     }
 
-    MPMI_STAMP(4);                                // horizon loop left (warp 0 of the CTA)
-    // ---- a5-a7 ------------------------------------------------------------------------------------
-    unsigned long long key = kKeyNone;
-    unsigned n_safe = 0, n_exec = 0;
+    if (blk == blockIdx.x) MPMI_STAMP(4);         // horizon loop left (warp 0 of the CTA, first batch)
+    // ---- a5 ------------------------------------------------------------------------------------------
     if (a.steps && q == 0 && li < ncand) a.steps[li] = steps;    // mpmi_step_trace
     if (q == 0 && li < ncand && inputs_ok) {
         const bool safe = steps == H;
@@ -134,10 +143,13 @@ rollout_lat_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ K
             const float df = __fsub_rn(z[D + j], u_h[j]);
             d2 = __fmaf_rn(df, df, d2);
         }
-        key = make_key(safe, d2, H, steps, cfg.shard_begin + li);
-        n_safe = safe ? 1u : 0u;
-        n_exec = (unsigned)(steps + 1 < H ? steps + 1 : H);
+        const unsigned long long kk = make_key(safe, d2, H, steps, cfg.shard_begin + li);
+        key = kk < key ? kk : key;
+        n_safe += safe ? 1u : 0u;
+        n_exec += (unsigned)(steps + 1 < H ? steps + 1 : H);
     }
+  }
+    // ---- a6 + a7 -------------------------------------------------------------------------------------
     block_select_and_finalise<kLatBlock / 32>(cfg, key, n_safe, n_exec, tick, u_h, a.st, a.out, a.partial, a.seq);
     MPMI_STAMP(5);                                // keys reduced, ticket taken (last CTA: result written)
 #undef MPMI_STAMP
