@@ -9,8 +9,8 @@ H-step rollout with per-step safe test -> argmin selection -> result, on one bat
 input (a fresh x0, u_user and Philox tick per step).  Default workload: C4 at N = 2^20, H = 100
 (BASELINE.json configs[3], the configuration the throughput half of the metric is quoted on).
 The rest of the metric rides on the same JSON line under "extra" (N = 1 only): the scale sweep
-N = 2^14 .. 2^20, C5 with a roofline of its own, the paper-scale latencies (C1, C2, C3) and the two
-HBM-bound trajectory dumps -- each with its own clock record.
+N = 2^14 .. 2^20, C5 with a roofline of its own, the paper-scale latencies (C1, C2, C3), the two
+HBM-bound trajectory dumps and the comparison rows (FP32-only, bare tensor-core, noise, re-lift, affine) -- each with its own clock record.
 
 value    = executed sample-steps/s with inputs resident in HBM (mpmi_step_device), CUDA-event timed
 e2e      = the same metric through mpmi_step_sync with HOST buffers (H2D + D2H inside the region)
@@ -360,6 +360,33 @@ def extra_c5(mp, args, local, flush, stream):
     return out
 
 
+def extra_variants(mp, args, local, flush, stream):
+    """the comparison rows of BASELINE.md's table (own metrics, not the headline): FP32-only ticks, the bare tensor-core kernel,
+    prediction noise, the re-lift model and the affine-in-u fast path -- a few ticks each, device-timed"""
+    import workloads as W
+    V = mp.mpmi
+    K_, W_ = 6, 3
+    rows = [("C4_fp32", "C4", V.VARIANT_NO_TENSOR, 0.0, 0), ("C4_bare_tensor_core", "C4", V.VARIANT_TC_UNVERIFIED, 0.0, 0),
+            ("C5_fp32", "C5", V.VARIANT_NO_TENSOR, 0.0, 0), ("C5_bare_tensor_core", "C5", V.VARIANT_TC_UNVERIFIED, 0.0, 0),
+            ("C4_noise_0.02", "C4", 0, 0.02, 0), ("C5_noise_0.01", "C5", 0, 0.01, 0), ("C4_relift", "C4", 0, 0.0, 1),
+            ("C4_affine", "C4", V.VARIANT_AFFINE, 0.0, 0), ("C5_affine", "C5", V.VARIANT_AFFINE, 0.0, 0)]
+    out = {}
+    with clocked(local) as ck:
+        for key, name, variant, sigma, relift in rows:
+            w = W.make(name)
+            w.noise_sigma = sigma; w.model_kind = relift
+            x0s, uus, ticks = W.tick_inputs(w, W_ + K_)
+            ctx = mp.Context(w, device=local, variant=variant)
+            m = measure_ticks(mp, ctx, w, x0s, uus, ticks, K_, W_, flush, stream)
+            info = ctx.info()
+            ms = float(m["step_ms"].sum())
+            out[key] = {"tick_ms": ms / K_, "sample_steps_per_s": m["n_exec"] / (ms * 1e-3), "kernel": KERNEL_NAMES.get(info["variant"], "?"),
+                        "launches_per_tick": info["launches_per_tick"]}
+            ctx.close()
+    out["clocks"] = ck.summary
+    return out
+
+
 def extra_latency(mp, args, local, stream):
     """paper-scale ticks (N ~ 1e4): host p50 / p99 of mpmi_step_sync; C2 replays its 1,000 stored closed-loop ticks"""
     import workloads as W
@@ -698,7 +725,7 @@ def main():
             lat.update(extra_latency(mp, args, local, stream))
         if not args.no_extras:
             extra = {"sweep": extra_sweep(mp, args, local, flush, stream), "C5": extra_c5(mp, args, local, flush, stream),
-                     "dumps": extra_dumps(mp, args, local, stream)}
+                     "dumps": extra_dumps(mp, args, local, stream), "variants": extra_variants(mp, args, local, flush, stream)}
 
     # ---- CPU baseline: the oracle as it stands on this box's host cores (bounded sample), then on one thread
     cpu = None
