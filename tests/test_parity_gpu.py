@@ -271,6 +271,33 @@ def test_spatial_binning_changes_nothing(mp, name, N):
             assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
 
 
+def test_binning_beyond_one_scan_pass_and_with_a_ragged_life_time_histogram(mp):
+    """Edges of the binning kernels: (a) more than 16,384 cells (2^21 candidates -> 2^15 cells), where the last CTA's scan of the cell
+    histogram takes a second pass and carries its running sum over; (b) a life-time histogram whose cell count H + 1 is not a multiple
+    of the scan's int4 groups, on few candidates (most CTA-level counters empty).  Both only re-order the walk: every field of the
+    result equals the unordered tick's."""
+    V = mp.mpmi
+    w = W.make("C4", N=(1 << 21) + 5)
+    plain = mp.Context(w, variant=V.VARIANT_NO_BINNING | V.VARIANT_NO_TENSOR)
+    binned = mp.Context(w, variant=V.VARIANT_NO_TENSOR)
+    assert binned.info()["binning_cells"] == 1 << 15 and plain.info()["binning_cells"] == 0
+    x0s, uus, ticks = W.tick_inputs(w, 2)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        a, b = plain.step_sync(x0, uu, int(t)).as_dict(w.m), binned.step_sync(x0, uu, int(t)).as_dict(w.m)
+        for k in ("index", "safe", "steps", "n_safe", "n_exec", "key", "dist"):
+            assert a[k] == b[k], (k, a[k], b[k])
+    plain.close(); binned.close()
+    w = W.make("C5", N=1500, H=37)                                # 38 life-time cells, two prediction CTAs
+    plain = mp.Context(w, variant=V.VARIANT_NO_BINNING)
+    pred = mp.Context(w, variant=V.VARIANT_FORCE_BINNING)
+    assert pred.info()["binning_cells"] == 38
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        a, b = plain.step_sync(x0, uu, int(t)).as_dict(w.m), pred.step_sync(x0, uu, int(t)).as_dict(w.m)
+        for k in ("index", "safe", "steps", "n_safe", "n_exec", "key", "dist"):
+            assert a[k] == b[k], (k, a[k], b[k])
+
+
 @pytest.mark.parametrize("name,N,noise,tensor", [("C5", 40000, 0.0, True), ("C5", 20000, 0.0, False), ("C5", 9000, 0.02, True)])
 def test_life_time_order_changes_nothing(mp, name, N, noise, tensor):
     """For the persistent tile kernels (d > 32) the pre-sort key is the first-violation step PREDICTED by the
