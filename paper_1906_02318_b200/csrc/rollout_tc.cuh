@@ -186,9 +186,11 @@ struct TcShared {
 // sigma * eps of Algorithm 2 l.5 for the tensor-core kernel: the state lives in the accumulator, so the
 // noise enters the contraction as 8 extra A columns [sigma eps_hi | sigma eps_lo] against the selector rows of the K_hi
 // image (1.0 at (r = j, c = D + 8 + j): exact in TF32, its lo part is 0): z'_j += sigma eps_j through two more MMAs per step.
+// Split in two so that the expensive half -- two Philox calls and three Box-Muller pairs per candidate and step, more than twice the
+// rest of a state warp's step -- runs AFTER the hand-back, while the tensor core works on this tile, and only the two stores stay
+// on the step's critical path.
 template <int D>
-__device__ __forceinline__ void tc_noise_store(const DevCfg &cfg, long long gi, int k, unsigned long long tick, uint32_t tlane) {
-    MPMI_TC_GEOM(D);
+__device__ __forceinline__ void tc_noise_compute(const DevCfg &cfg, long long gi, int k, unsigned long long tick, float (&v)[8]) {
     float g[8];                                                  // eps of the ORIGINAL dims 0..7
 #pragma unroll
     for (int q = 0; q < 2; q++) {
@@ -197,13 +199,16 @@ __device__ __forceinline__ void tc_noise_store(const DevCfg &cfg, long long gi, 
 #pragma unroll
         for (int e = 0; e < 4; e++) g[4 * q + e] = g4[e];
     }
+#pragma unroll
+    for (int j = 0; j < 8; j++)                                  // internal dim j = original dim perm[j]
+        v[j] = j < cfg.n ? __fmul_rn(cfg.noise_sigma, g[cfg.perm[j] & 7]) : 0.f;
+}
+template <int D>
+__device__ __forceinline__ void tc_noise_put(const float (&v)[8], uint32_t tlane) {
+    MPMI_TC_GEOM(D);
     uint32_t nh[8], nl[8];
 #pragma unroll
-    for (int j = 0; j < 8; j++) {                                // internal dim j = original dim perm[j]
-        const float v = j < cfg.n ? __fmul_rn(cfg.noise_sigma, g[cfg.perm[j] & 7]) : 0.f;
-        nh[j] = __float_as_uint(v);
-        nl[j] = tf32_lo(v);
-    }
+    for (int j = 0; j < 8; j++) { nh[j] = __float_as_uint(v[j]); nl[j] = tf32_lo(v[j]); }
     tc::tmem_st8(tlane + kTcColNhi, nh);
     tc::tmem_st8(tlane + kTcColNlo, nl);
 }
@@ -410,6 +415,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                 }
             }
             __syncwarp();                                                // tcgen05.st / ld below are .sync.aligned
+            float nz[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};      // NOISE: sigma * eps of the next MMA step (internal dims 0..7)
             {
                 float x[kMaxN];
                 if (!shared_x0) {
@@ -442,11 +448,16 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     if (lane == 0) sh.warp_alive[q] = any ? 1u : 0u;
                 }
                 if (NOISE && hc == kTcStateWarps / 4 - 1)          // the last column group draws the noise of step 0
-                    tc_noise_store<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, 0, tick, tlane);
+                {
+                    tc_noise_compute<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, 0, tick, nz);
+                    tc_noise_put<D>(nz, tlane);
+                }
             }
             wait_st();
             fence_before_sync();
             mbar_arrive(bar_alo);
+            if (NOISE && hc == kTcStateWarps / 4 - 1 && H > 1)           // noise of MMA step 1, while step 0 runs
+                tc_noise_compute<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, 1, tick, nz);
 
             // ---- a3 + a4: after MMA step s-1 the accumulator holds z_s; test it, split it, hand it back
             int s = 1;
@@ -491,7 +502,7 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                         tmem_st8(tlane + kTcColAlo + c0 + cc, lo);
                     }
                     if (NOISE && hc == kTcStateWarps / 4 - 1)      // noise of MMA step s (it produces z_{s+1})
-                        tc_noise_store<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, s, tick, tlane);
+                        tc_noise_put<D>(nz, tlane);                  // (computed after the previous hand-back)
                 }
                 if (dump && li < ncand) {                                // a9: traj[(k*J + row)*Ncand + i], k = s-1
 #pragma unroll
@@ -509,6 +520,8 @@ rollout_tc_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KA
                     mbar_arrive(bar_alo);
                     SWT(sw_st);
                 }
+                if (NOISE && hc == kTcStateWarps / 4 - 1 && s + 1 < H)   // noise of MMA step s + 1, while step s runs
+                    tc_noise_compute<D>(cfg, (MODE == MODE_TICK ? cfg.shard_begin : 0) + li, s + 1, tick, nz);
                 if (verify && hc == 0) {                                 // off the step's critical path: after the hand-back
                     float x[NB];
 #pragma unroll
