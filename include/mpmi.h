@@ -76,8 +76,8 @@ enum { MPMI_VARIANT_NARROW = 1,         /* 2 candidates per thread (latency)    
                                            constant-memory slots of its device are taken                      */
        MPMI_VARIANT_TC_UNVERIFIED = 4096, /* tensor-core kernels WITHOUT the verification below: the bare 3xTF32
                                            rollout (benchmark / test knob -- its flags are only as good as T1) */
-       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32: take the tensor-core tick below 2^16 candidates too   */
-/* The tensor-core tick (default at padded d = 128, and at padded d = 32 from 2^16 candidates; linear model) is VERIFIED:
+       MPMI_VARIANT_TENSOR32 = 1024 };  /* padded d = 32: take the tensor-core tick for small candidate sets too */
+/* The tensor-core tick (default at padded d = 128, and at padded d = 32 above 256 candidates per SM, ~38,000; linear model) is VERIFIED:
  * the 3xTF32 tcgen05 kernel rolls all candidates; every candidate whose state came within tau_i(k) of a safe-set
  * boundary is rolled again by the FP32 kernel (register kernel at d = 32, warp-tile kernel at d = 128), which merges
  * its keys and finalises, so that flags and winner are those of the FP32 tick.  tau_i(k) is a per-tick, per-step,
@@ -166,7 +166,7 @@ typedef struct {
     int32_t  d_pad;           /* internal padded lifted dim (zero rows / columns: exact)            */
     int32_t  variant;         /* 1 = register-resident FFMA2 (d<=32), 2 = warp-tile FFMA2 (d<=128),
                                  3 = latency kernel, 4 lanes per candidate (d<=32, small N),
-                                 4 = verified 3xTF32 tcgen05 tensor-core tick (d_pad = 128; d_pad = 32 from 2^16 candidates),
+                                 4 = verified 3xTF32 tcgen05 tensor-core tick (d_pad = 128; d_pad = 32 above 256 candidates per SM),
                                  5 = re-lift kernel (MPMI_MODEL_RELIFT), 6 = affine-in-u kernel       */
     int32_t  cand_per_block, threads_per_block, blocks, smem_bytes, regs_per_thread;
     int32_t  sm_count, launches_per_tick, uses_graph;

@@ -122,7 +122,10 @@ namespace {
 
 constexpr unsigned kProfRing = 64;
 constexpr long long kLatMaxCand = 24576;        // <= this many candidates: latency kernel (measured: 125 vs 155 us at 2^14, 210 vs 164 us at 2^15)
-constexpr long long kTc32MinCand = 1LL << 16;   // D = 32: tensor-core kernel from this many candidates (four CTAs per SM need >= 592 tiles to fill)
+// D = 32: the verified tensor-core tick takes over where the register kernel needs a second CTA on an SM (256 candidates per CTA: its tick
+// then doubles, 157 -> 273 us on 148 SMs; the tensor-core tick without binning: 177 us at 40,000 candidates, 193 us at 2^16); its binning
+// pays from ~80,000 candidates (2^16: 193 us without, 204 us with; 98,304: 256 / 234 us)
+constexpr long long kTc32CandPerCta = 256, kTc32MinBinning = 81920;
 
 thread_local std::string g_create_err;
 
@@ -652,9 +655,9 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         const long long send = sb + sc < cfg->N ? sb + sc : cfg->N;
         const long long nsamp = send > sb ? send - sb : 0;
         // measured at d = 32: the ~25 us of binning pay from 2^17 candidates for the register kernel (a warp of 64 candidates), from
-        // 2^16 for the tensor-core tick (a tile of 128 candidates runs until its last one stops)
+        // ~80,000 for the tensor-core tick (a tile of 128 candidates runs until its last one stops)
         const bool tc32 = D == 32 && tc_model_ok && cfg->model == MPMI_MODEL_LINEAR;
-        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (D > 32 ? (1 << 15) : tc32 ? (1 << 16) : (1 << 17));
+        const bool want = cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= (D > 32 ? (1 << 15) : tc32 ? kTc32MinBinning : (1 << 17));
         c->binning = (cfg->variant & MPMI_VARIANT_FORCE_BINNING) ? (cfg->sampler == MPMI_SAMPLER_PHILOX && nsamp >= 64)
                                                                   : (want && !(cfg->variant & MPMI_VARIANT_NO_BINNING));
         if (c->binning) {
@@ -726,7 +729,7 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         }
         // D = 32, large candidate sets: the 3xTF32 tcgen05 kernel of d = 128 with N = 32 MMAs and four CTAs per SM, as a
         // VERIFIED tick (below).  The batch entry stays on the FP32 register kernels chosen above.
-        if (D == 32 && c->variant == 1 && tc_model_ok && (sc >= kTc32MinCand || (cfg->variant & MPMI_VARIANT_TENSOR32)) &&
+        if (D == 32 && c->variant == 1 && tc_model_ok && (sc > kTc32CandPerCta * c->sm_count || (cfg->variant & MPMI_VARIANT_TENSOR32)) &&
             !(cfg->variant & (MPMI_VARIANT_NARROW | MPMI_VARIANT_WIDE | MPMI_VARIANT_LATENCY | MPMI_VARIANT_SMEM_MODEL))) {
             tensor = true;
             c->variant = 4;

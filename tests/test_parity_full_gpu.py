@@ -236,7 +236,7 @@ def _verified_cases():
 
 @pytest.mark.parametrize("case", ["C4_full", "C5_full", "C5_x100", "C5_x1000", "C4_off_origin_30", "C4_off_origin_100", "C4_noise", "C5_noise"])
 def test_verified_tick_equals_fp32_tick_every_candidate(mp, case):
-    """The verified tensor-core tick (default at padded d = 128, and at d = 32 from 2^16 candidates) must reproduce the FP32
+    """The verified tensor-core tick (default at padded d = 128, and at d = 32 above 256 candidates per SM) must reproduce the FP32
     tick candidate by candidate: every step count, hence every flag, and the winner --
     at the sizes bench.py times, with the state scaled up 100x and 1000x against the absolute margin, with the annulus far
     from the origin, and with prediction noise.  The second pass must stay a small fraction of the candidates."""

@@ -370,7 +370,7 @@ def _same_tick(a, b):
 
 
 def test_verified_tensor_core_tick_d32(mp):
-    """The default tick at padded d = 32 from 2^16 candidates: the 3xTF32 tcgen05 kernel (N = 32 MMAs, four CTAs per SM) as a
+    """The default tick at padded d = 32 from ~38,000 candidates (more than one register-kernel CTA per SM): the 3xTF32 tcgen05 kernel (N = 32 MMAs, four CTAs per SM) as a
     VERIFIED tick.  Every candidate whose 3xTF32 state came within tau_i(k) (csrc/bound.cuh: a per-tick bound, derived from the
     model, on the difference to the FP32 rollout) of the safe-set boundary is rolled again by the FP32 register kernel, which
     merges its keys and finalises.  Checked: T3 against the oracle, and -- the strong one -- the SAME result (index, safe, steps,
@@ -385,7 +385,9 @@ def test_verified_tensor_core_tick_d32(mp):
     assert info["variant"] == 4 and info["threads_per_block"] == 160 and info["blocks"] == 4 * info["sm_count"]
     assert info["launches_per_tick"] == 6                                # hist, scatter | bound x2 -> tcgen05 rollout -> FP32 second pass
     assert fp32.info()["variant"] == 1
-    assert mp.Context(W.make("C4", N=(1 << 16) - 2)).info()["variant"] == 1                       # below the crossover: FP32
+    assert mp.Context(W.make("C4", N=30000)).info()["variant"] == 1                               # below the crossover (one register-kernel CTA per SM): FP32
+    small = mp.Context(W.make("C4", N=50000)).info()
+    assert small["variant"] == 4 and small["binning_cells"] == 0 and small["launches_per_tick"] == 4   # above it: verified tick, binning only from ~80,000
     assert mp.Context(W.make("C4", N=1 << 15), variant=V.VARIANT_TENSOR32).info()["variant"] == 4  # ... unless asked for
     o = _oracle(w)
     H = w.H
