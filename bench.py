@@ -568,7 +568,7 @@ def main():
                     help="BASELINE.json configs[3] alone: N = 2^14 .. 2^20 on the C4 model, sample-steps/s and tick latency at each N")
     ap.add_argument("--affine", action="store_true",
                     help="affine-in-u fast path x_k = a_k + G_k u (SURVEY 8(f) NEXT-4): same selections, n*m FMAs per sample-step; its own metric")
-    ap.add_argument("--tensor32", action="store_true", help="d = 32: take the verified tensor-core tick below 2^16 candidates too (it is the default from 2^16)")
+    ap.add_argument("--tensor32", action="store_true", help="d = 32: take the verified tensor-core tick for small candidate sets too (it is the default above 256 candidates per SM)")
     ap.add_argument("--unverified", action="store_true", help="tensor-core kernels without the verification pass (measurement only: the bare 3xTF32 rollout)")
     ap.add_argument("--no-predict", action="store_true", help="d > 32: pre-sort by input-box cell instead of by predicted life time")
     ap.add_argument("--no-tensor", action="store_true", help="FP32 kernels only (d = 32: register kernel, d = 128: SIMT warp-tile kernel)")
