@@ -21,4 +21,4 @@ static KernFn pick_m(int M) {
     return nullptr;
 }
 // rs = lanes per candidate pair (2 or 4)
-KernFn FN(int M, int rs) { return rs == 2 ? pick_m<2>(M) : rs == 4 ? pick_m<4>(M) : nullptr; }
+KernFn FN(int M, int rs) { return rs == 2 ? pick_m<2>(M) : rs == 4 ? pick_m<4>(M) : rs == 8 ? pick_m<8>(M) : nullptr; }

@@ -848,11 +848,13 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
         if (D == 32) {               // FP32 register kernel, 2 candidates per thread, CTAs loop over blocks of the lists
             const int rc_kconst = (c->kslot >= 0 && !std::getenv("MPMI_RC_SMEM")) ? 1 : 0;
             c->k_recheck = noise ? mpmi_pick_regn_32_recheck(M, rc_kconst) : mpmi_pick_reg_32_recheck(M, rc_kconst);
-            // lanes per candidate pair in the second pass (measured, rollout_split.cuh): 4 up to 2^19 candidates, 2 beyond
+            // lanes per candidate pair in the second pass (measured, rollout_split.cuh): the fewer deferred candidates, the more the pass
+            // is one warp's chain over the horizon -- 8 lanes up to ~300,000 candidates (40,000: tick 180 -> 164 us against 4 lanes, 2^16:
+            // 192 -> 176, 2^17: 266 -> 255, 2^18: 376 -> 369, 2^19: 603 -> 620), 4 up to 2^19, 2 beyond
             // (0: one thread per pair, rollout_reg_kernel -- when the shared-memory model is forced, or MPMI_RC_RS=0)
-            int rc_rs = sc <= (1LL << 19) ? 4 : 2;
+            int rc_rs = sc <= 300000 ? 8 : sc <= (1LL << 19) ? 4 : 2;
             if (const char *e = std::getenv("MPMI_RC_RS")) rc_rs = std::atoi(e);
-            if (rc_rs == 2 || rc_rs == 4) {
+            if (rc_rs == 2 || rc_rs == 4 || rc_rs == 8) {
                 // row-split kernel, one-warp CTAs rolling blocks of 64 / RS candidates, 8 per SM: the pass is set by how long ONE
                 // warp needs for the horizon, and RS lanes per pair cut that RS-fold (measured on C4, 3.8 % of 2^20 candidates:
                 // one thread per pair 250 us however the blocks are dealt out)
