@@ -271,6 +271,22 @@ def test_spatial_binning_changes_nothing(mp, name, N):
             assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
 
 
+@pytest.mark.parametrize("N,lanes", [(45000, 8), (400000, 4), (600000, 2)])
+def test_every_lane_split_of_the_d32_second_pass(mp, N, lanes):
+    """The row-split second pass runs 8, 4 or 2 lanes per candidate pair depending on the candidate count (mpmi_api.cu: rc_rs); each
+    form must leave the verified tick identical to the FP32 tick (N = 45,000 also: the verified tick WITHOUT binning)."""
+    V = mp.mpmi
+    w = W.make("C4", N=N)
+    ver, fp32 = mp.Context(w), mp.Context(w, variant=V.VARIANT_NO_TENSOR)
+    assert ver.info()["variant"] == 4 and fp32.info()["variant"] == 1
+    assert (ver.info()["binning_cells"] > 0) == (N >= 81920)
+    x0s, uus, ticks = W.tick_inputs(w, 3)
+    for x0, uu, t in zip(x0s, uus, ticks):
+        a, b = ver.step_sync(x0, uu, int(t)).as_dict(w.m), fp32.step_sync(x0, uu, int(t)).as_dict(w.m)
+        assert _same_tick(a, b), (lanes, a, b)
+        assert ver.info()["reserved"] > 0                      # some candidates did go through the second pass
+
+
 def test_binning_beyond_one_scan_pass_and_with_a_ragged_life_time_histogram(mp):
     """Edges of the binning kernels: (a) more than 16,384 cells (2^21 candidates -> 2^15 cells), where the last CTA's scan of the cell
     histogram takes a second pass and carries its running sum over; (b) a life-time histogram whose cell count H + 1 is not a multiple
