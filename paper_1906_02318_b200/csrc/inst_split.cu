@@ -20,5 +20,5 @@ static KernFn pick_m(int M) {
     }
     return nullptr;
 }
-// rs = lanes per candidate pair (2 or 4)
-KernFn FN(int M, int rs) { return rs == 2 ? pick_m<2>(M) : rs == 4 ? pick_m<4>(M) : rs == 8 ? pick_m<8>(M) : nullptr; }
+// rs = lanes per candidate pair (2, 4, 8 or 16)
+KernFn FN(int M, int rs) { return rs == 2 ? pick_m<2>(M) : rs == 4 ? pick_m<4>(M) : rs == 8 ? pick_m<8>(M) : rs == 16 ? pick_m<16>(M) : nullptr; }

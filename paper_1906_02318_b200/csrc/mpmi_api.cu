@@ -852,9 +852,9 @@ int mpmi_create(const mpmi_config *cfg, mpmi_ctx **out) {
             // is one warp's chain over the horizon -- 8 lanes up to ~300,000 candidates (40,000: tick 180 -> 164 us against 4 lanes, 2^16:
             // 192 -> 176, 2^17: 266 -> 255, 2^18: 376 -> 369, 2^19: 603 -> 620), 4 up to 2^19, 2 beyond
             // (0: one thread per pair, rollout_reg_kernel -- when the shared-memory model is forced, or MPMI_RC_RS=0)
-            int rc_rs = sc <= 300000 ? 8 : sc <= (1LL << 19) ? 4 : 2;
+            int rc_rs = sc <= 80000 ? 16 : sc <= 300000 ? 8 : sc <= (1LL << 19) ? 4 : 2;     // (16: 40,000 candidates 164 -> 157 us, 2^16 176 -> 173 us)
             if (const char *e = std::getenv("MPMI_RC_RS")) rc_rs = std::atoi(e);
-            if (rc_rs == 2 || rc_rs == 4 || rc_rs == 8) {
+            if (rc_rs == 2 || rc_rs == 4 || rc_rs == 8 || rc_rs == 16) {
                 // row-split kernel, one-warp CTAs rolling blocks of 64 / RS candidates, 8 per SM: the pass is set by how long ONE
                 // warp needs for the horizon, and RS lanes per pair cut that RS-fold (measured on C4, 3.8 % of 2^20 candidates:
                 // one thread per pair 250 us however the blocks are dealt out)

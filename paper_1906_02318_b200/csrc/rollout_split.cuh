@@ -4,7 +4,7 @@
 // rollout_reg_kernel gives one thread a whole candidate pair: D (D + M) = 1088 dependent-issue FFMA2 per step, ~2,200 clk of a
 // sub-partition's FMA pipe.  That is the right shape when the grid fills the machine several times over, but the second pass sees
 // a few per cent of the candidates -- about one such warp per sub-partition -- and then lasts as long as ONE warp needs for the
-// whole horizon (measured on C4: 250 us for 3.8 % of 2^20 candidates, however the blocks are dealt out).  Here RS = 2, 4 or 8
+// whole horizon (measured on C4: 250 us for 3.8 % of 2^20 candidates, however the blocks are dealt out).  Here RS = 2, 4, 8 or 16
 // consecutive lanes share a candidate pair: lane q owns rows [q D/RS, (q+1) D/RS) of z' = K z + B u for
 // both candidates of the pair (FFMA2, model value broadcast to both halves, from shared memory: the lanes of a warp need different
 // rows, so the constant-bank operand of rollout_reg_kernel does not apply), then the RS lanes all-gather the new state with warp
@@ -17,6 +17,8 @@
 // and is slightly slower: second pass 0.197 -> 0.212 ms at 2^20 candidates, 0.104 -> 0.108 ms at 2^18.)
 // With 8 lanes per pair (4 rows per lane) the chain halves again: best up to ~300,000 candidates (tick at 40,000 / 2^16 / 2^17 / 2^18
 // candidates 164 / 176 / 255 / 369 us against 180 / 192 / 266 / 376 us with 4 lanes).
+// 16 lanes (one row pair per lane) still gain below ~80,000 candidates (40,000: 157 against 164 us, 2^16: 173 against 176 us; 100,000:
+// 223 against 221 us): the all-gather's 64 shuffles per step do not shrink with the rows.
 // (Round-2 late: FFMA2 over two ROWS of one candidate instead of one row of two candidates removed ~1.5 register moves per FFMA2
 // -- the pass was bound by issue slots: second pass at 2^20 candidates 0.198 -> 0.166 ms, verified tick at 2^16 .. 2^20 now
 // 208 / 263 / 376 / 596 / 964 us.)
@@ -35,7 +37,7 @@ constexpr int kSplitBlock = 128;
 template <int D, int M, int RS, bool NOISE = false>
 __global__ void __launch_bounds__(kSplitBlock, 3)
 rollout_split_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__ KArgs a) {
-    static_assert(D == 32 && (RS == 2 || RS == 4 || RS == 8), "row-split kernel: D = 32; 2, 4 or 8 lanes per candidate pair");
+    static_assert(D == 32 && (RS == 2 || RS == 4 || RS == 8 || RS == 16), "row-split kernel: D = 32; 2, 4, 8 or 16 lanes per candidate pair");
     constexpr int RL = D / RS;                   // rows per lane
     constexpr int NB = kMaxN;
     __shared__ __align__(16) float sK[(D + M) * D];
@@ -102,8 +104,14 @@ rollout_split_kernel(const __grid_constant__ DevCfg cfg, const __grid_constant__
             for (int cc = 0; cc < D + M; cc++) {                 // columns descending, as in rollout_reg_kernel
                 const int c = D + M - 1 - cc;
                 const float2 zc = z[c];
+                if (RL == 2) {                               // 16 lanes per pair: one row pair per lane
+                    float2 k01;
+                    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(k01.x), "=f"(k01.y) : "r"(sbase + (unsigned)(c * D * 4)));
+                    if (cc == 0) { mul2_bcast_z(acc0[0], k01, zc.x); mul2_bcast_z(acc1[0], k01, zc.y); }
+                    else         { fma2_bcast_z(acc0[0], k01, zc.x); fma2_bcast_z(acc1[0], k01, zc.y); }
+                }
 #pragma unroll
-                for (int r = 0; r < RL; r += 4) {
+                for (int r = 0; r + 3 < RL; r += 4) {
                     const float4 kv = lds128(sbase + (c * D + r) * 4);
                     const float2 k01 = make_float2(kv.x, kv.y), k23 = make_float2(kv.z, kv.w);
                     if (cc == 0) {

@@ -271,9 +271,9 @@ def test_spatial_binning_changes_nothing(mp, name, N):
             assert accept_selection(b, o.step(x0, uu, int(t), detail=True), w.H)[0]
 
 
-@pytest.mark.parametrize("N,lanes", [(45000, 8), (400000, 4), (600000, 2)])
+@pytest.mark.parametrize("N,lanes", [(45000, 16), (150000, 8), (400000, 4), (600000, 2)])
 def test_every_lane_split_of_the_d32_second_pass(mp, N, lanes):
-    """The row-split second pass runs 8, 4 or 2 lanes per candidate pair depending on the candidate count (mpmi_api.cu: rc_rs); each
+    """The row-split second pass runs 16, 8, 4 or 2 lanes per candidate pair depending on the candidate count (mpmi_api.cu: rc_rs); each
     form must leave the verified tick identical to the FP32 tick (N = 45,000 also: the verified tick WITHOUT binning)."""
     V = mp.mpmi
     w = W.make("C4", N=N)
